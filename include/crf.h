@@ -1,0 +1,155 @@
+/* crf.h -- C ABI of libcrf.so: pointwise thermochemistry and mixture-averaged transport
+ * for reactive low-Mach flow (the data-parallel hot path of arXiv 2409.06404, nekCRF),
+ * evaluated by hand-written sm_100a CUDA kernels.
+ *
+ * What the calls compute.  The paper's right-hand-side function "employs highly optimized
+ * kernels for ... species production rates, and thermodynamic and transport properties"
+ * generated from "a combustion model expressed in Cantera format"; the
+ * quantities are the ones Eq. 1a-1d consume (omega_k, h_k, c_p, lambda, rho)
+ * and the mixture-averaged D_k of Eq. 2 and mu of Eq. 4.  The
+ * paper prints none of the formulas; the definitions are the Chemkin-II/Cantera ones in the
+ * reading of SURVEY.md section 8(c), restated in DESIGN.md "What the path computes".
+ *
+ * Conventions (all calls).
+ *  - SI units with kmol.  R = 8314.46261815324 J/(kmol K).
+ *  - Field arguments are DEVICE pointers owned by the caller, except in crf_step_host.
+ *    T[n], p[n]: temperature [K] and thermodynamic pressure [Pa] per point.
+ *    Y[Ns*n]: mass fractions, species-major: Y[k*n + i] (one contiguous field per species,
+ *    the element-lexicographic field layout of PAPER.md:213).  Y carries all Ns species
+ *    (the caller fills the excess species); it is used as given: never
+ *    clipped, never renormalised.
+ *  - Every pointer must be 16-byte aligned; inputs must not alias outputs.  n >= 0 is the
+ *    number of points; n = 0 is a no-op.  Odd n is accepted (scalar tail).
+ *  - Calls are asynchronous on the mechanism's stream (crf_mech_set_stream, default: the
+ *    legacy default stream) and do not synchronise.
+ *  - Return 0 (CRF_OK) or a negative code; crf_last_error() gives the text of the last
+ *    failure on the calling thread.  Non-finite or unphysical inputs (T <= 0) are not
+ *    checked; outputs are then unspecified.  No C++ exception crosses this boundary.
+ */
+#ifndef CRF_H
+#define CRF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CRF_OK 0
+#define CRF_EINVAL (-1)       /* null or misaligned pointer, negative n, inconsistent tables */
+#define CRF_EUNSUPPORTED (-2) /* mechanism too large for the compiled kernels */
+#define CRF_ECUDA (-3)        /* CUDA allocation/launch failure (text in crf_last_error) */
+
+#define CRF_TABLES_VERSION 1
+#define CRF_MAX_SLOTS 3 /* reactant (and product) slots per reaction */
+
+/* Host-side species-major SoA mechanism tables, produced by the packer
+ * (paper_2409_06404_b200/packer.py) from a mechanism description.  All pointers are HOST
+ * pointers; crf_mech_create copies what it needs, the caller may free them afterwards.
+ *
+ * Reactions are sorted by type: [0, Nr-N3-Nt) elementary, then N3 third-body, then Nt Troe
+ * falloff.  Rate constants are in SI-kmol units and stored as logarithms:
+ * k = exp(lnA + beta ln T - Ea_R / T).  All reactions are reversible; the reverse constant
+ * is k_f / K_c with K_c = exp(-sum_k nu_k g_k/(RT)) (p_ref/(RT))^dnu. */
+typedef struct crf_tables {
+    int32_t version; /* CRF_TABLES_VERSION */
+    int32_t Ns;      /* species */
+    int32_t Nr;      /* reactions */
+    int32_t N3;      /* third-body reactions (both rates of progress multiplied by [M]) */
+    int32_t Nt;      /* Troe falloff reactions */
+    int32_t reserved;
+    double p_ref; /* Pa: standard pressure of the NASA entropies and of the D_jk fits */
+
+    const double *W;       /* [Ns]    molar mass, kg/kmol */
+    const double *Tmid;    /* [Ns]    NASA range switch: T <= Tmid uses nasa_lo */
+    const double *nasa_lo; /* [7][Ns] a1..a7, coefficient-major: nasa_lo[c*Ns + k] */
+    const double *nasa_hi; /* [7][Ns] */
+
+    const double *lnA;  /* [Nr] (falloff: high-pressure limit) */
+    const double *beta; /* [Nr] */
+    const double *Ea_R; /* [Nr] K */
+    const int16_t *reac; /* [CRF_MAX_SLOTS][Nr] reactant species per slot, -1 = empty;
+                            a species listed twice has stoichiometric coefficient 2 */
+    const int16_t *prod; /* [CRF_MAX_SLOTS][Nr] product species per slot */
+
+    /* third-body efficiencies, CSR over the N3+Nt reactions that have a third body, in the
+     * sorted order: [M]_r = sum_k C_k + sum_{e in row r} eff_val[e] * C_{eff_idx[e]},
+     * eff_val = efficiency - 1 */
+    const int32_t *eff_ptr; /* [N3+Nt+1] */
+    const int16_t *eff_idx; /* [eff_ptr[N3+Nt]] */
+    const double *eff_val;  /* [eff_ptr[N3+Nt]] */
+
+    /* Troe falloff, one entry per falloff reaction: low-pressure limit k0 and
+     * F_cent = (1-alpha) exp(-T/T3) + alpha exp(-T/T1) + exp(-T2/T) */
+    const double *lnA0, *beta0, *Ea0_R, *alpha, *T3, *T1, *T2; /* [Nt] each */
+
+    /* transport fits, natural-log cubics in ln T: ln f = c[0] + c[1] x + c[2] x^2 + c[3] x^3 */
+    const double *mu_c;  /* [4][Ns]            ln(mu_k / Pa s) */
+    const double *lam_c; /* [4][Ns]            ln(lambda_k / (W/m/K)) */
+    const double *D_c;   /* [4][Ns(Ns+1)/2]    ln(D_jk / (m^2/s)) at p_ref, upper triangle incl.
+                            the diagonal, pair (j <= k) at j*Ns - j(j-1)/2 + (k - j) */
+} crf_tables;
+
+typedef struct crf_mech crf_mech; /* opaque; owns the device copies of all tables */
+
+/* Builds the device-resident mechanism (tables re-laid-out for the kernels and uploaded to
+ * the current CUDA device).  Returns CRF_EINVAL for inconsistent tables (bad version, species
+ * index out of range, no reactant, W <= 0 ...), CRF_EUNSUPPORTED if Ns exceeds what the
+ * kernels support (512), CRF_ECUDA on allocation failure.  *out is set only on success. */
+int crf_mech_create(const crf_tables *tables, crf_mech **out);
+void crf_mech_destroy(crf_mech *mech);
+
+/* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default. */
+int crf_mech_set_stream(crf_mech *mech, void *cuda_stream);
+int crf_mech_num_species(const crf_mech *mech);
+int crf_mech_num_reactions(const crf_mech *mech);
+
+/* NASA-7 mixture thermodynamics (c_p and h_k of Eq. 1b).
+ *   cp[n]  mixture heat capacity  sum_k Y_k c_{p,k}/W_k          [J/(kg K)]
+ *   h[n]   mixture enthalpy       sum_k Y_k h_k/W_k              [J/kg]
+ * p is accepted for uniformity and not read (may be NULL). */
+int crf_thermo(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
+               double *cp, double *h);
+
+/* Per-species molar properties (the c_{p,k}, h_k of Eq. 1b): cpk, hk, sk are [Ns*n] species-major,
+ * J/(kmol K), J/kmol, J/(kmol K); any of the three may be NULL. */
+int crf_thermo_species(const crf_mech *mech, const double *T, int64_t n, double *cpk, double *hk, double *sk);
+
+/* Net molar production rates from finite-rate chemistry and the heat release
+ * (omega_k of Eq. 1a and the source of Eq. 1b).
+ *   omega[Ns*n]  sum_r nu_kr (Q_f - Q_r)       [kmol/(m^3 s)], species-major
+ *   qdot[n]      -sum_k h_k(T) omega_k          [W/m^3], positive when exothermic */
+int crf_production_rates(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
+                         double *omega, double *qdot);
+
+/* Mixture-averaged transport (lambda of Eq. 1b, D_k of Eq. 2,
+ * mu of Eq. 4).
+ *   mu[n]        Wilke mixture viscosity                                   [Pa s]
+ *   lambda[n]    (sum X_k lambda_k + 1/sum X_k/lambda_k)/2                 [W/(m K)]
+ *   rhoD[Ns*n]   rho D_km, D_km = (1 - Y_k)/sum_{j!=k} X_j/D_jk, D_jk ~ p_ref/p; a pure
+ *                species (sum exactly 0) gives rho D_kk                    [kg/(m s)] */
+int crf_mix_transport(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
+                      double *mu, double *lambda, double *rhoD);
+
+/* One pass of the whole path with HOST buffers: copies T, p, Y to the device in chunks, runs
+ * crf_thermo, crf_production_rates and crf_mix_transport on each chunk and copies the seven
+ * outputs back, chunks pipelined over internal streams.  All pointers are host pointers with
+ * the layouts above (species-major with leading dimension n); pinned memory gives full copy
+ * bandwidth.  Synchronous: returns when every output is in host memory. */
+int crf_step_host(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
+                  double *cp, double *h, double *omega, double *qdot, double *mu, double *lambda, double *rhoD);
+
+/* Sustained FP64 pipe rate of the current device: runs a register-only kernel of `iters`
+ * dependent-chain DFMA groups on every SM and returns the FP64 instructions per second it
+ * reached in *inst_per_s (the measured denominator of the ALU roofline).  Synchronous. */
+int crf_fp64_probe(int iters, double *inst_per_s);
+
+/* How many kernel launches this library has issued in this process (for bench.py). */
+int64_t crf_launch_count(void);
+
+const char *crf_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CRF_H */

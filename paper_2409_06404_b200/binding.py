@@ -1,0 +1,155 @@
+"""Thin ctypes binding of libcrf.so (include/crf.h).  Argument marshalling only: every step of
+the path runs in the CUDA kernels of ``csrc/``.  PyTorch supplies device memory and streams.
+
+There is no CPU fallback: if ``libcrf.so`` is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+from . import packer
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcrf.so")
+_lib = None
+
+EXPORTS = ("crf_mech_create", "crf_mech_destroy", "crf_mech_set_stream", "crf_mech_num_species",
+           "crf_mech_num_reactions", "crf_thermo", "crf_thermo_species", "crf_production_rates",
+           "crf_mix_transport", "crf_step_host", "crf_fp64_probe", "crf_launch_count", "crf_last_error")
+
+
+class CrfError(RuntimeError):
+    pass
+
+
+def lib() -> C.CDLL:
+    """Loads libcrf.so (built in-tree by ``build.py``); raises if it is not there."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise CrfError(f"{LIB_PATH} not found: run `python -m paper_2409_06404_b200.build` "
+                           "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, dp = C.c_void_p, C.c_int64, C.c_void_p
+        L.crf_mech_create.argtypes = [C.POINTER(packer.CrfTables), C.POINTER(vp)]
+        L.crf_mech_destroy.argtypes = [vp]
+        L.crf_mech_destroy.restype = None
+        L.crf_mech_set_stream.argtypes = [vp, vp]
+        L.crf_mech_num_species.argtypes = [vp]
+        L.crf_mech_num_reactions.argtypes = [vp]
+        L.crf_thermo.argtypes = [vp, dp, dp, dp, i64, dp, dp]
+        L.crf_thermo_species.argtypes = [vp, dp, i64, dp, dp, dp]
+        L.crf_production_rates.argtypes = [vp, dp, dp, dp, i64, dp, dp]
+        L.crf_mix_transport.argtypes = [vp, dp, dp, dp, i64, dp, dp, dp]
+        L.crf_step_host.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
+        L.crf_fp64_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
+        L.crf_launch_count.restype = C.c_int64
+        L.crf_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(code: int):
+    if code != 0:
+        raise CrfError(f"libcrf error {code}: {lib().crf_last_error().decode()}")
+
+
+def launch_count() -> int:
+    return int(lib().crf_launch_count())
+
+
+def fp64_probe(iters: int = 4096) -> float:
+    """Measured sustained FP64 instructions/s of the current device (crf_fp64_probe)."""
+    out = C.c_double()
+    _check(lib().crf_fp64_probe(int(iters), C.byref(out)))
+    return out.value
+
+
+def _dev(t: torch.Tensor | None, shape=None):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise CrfError("expected a contiguous float64 CUDA tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise CrfError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return t.data_ptr()
+
+
+def _host(t: torch.Tensor, shape):
+    if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+        raise CrfError(f"expected a contiguous float64 host tensor of shape {tuple(shape)}")
+    return t.data_ptr()
+
+
+class Mechanism:
+    """Device-resident mechanism (``crf_mech``).  ``mech`` is a description dict or PackedTables."""
+
+    def __init__(self, mech):
+        self.tables = mech if isinstance(mech, packer.PackedTables) else packer.pack(mech)
+        self.Ns, self.Nr = self.tables.Ns, self.tables.Nr
+        handle = C.c_void_p()
+        struct = self.tables.as_struct()
+        _check(lib().crf_mech_create(C.byref(struct), C.byref(handle)))
+        self._h = handle
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().crf_mech_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _sync_stream(self):
+        _check(lib().crf_mech_set_stream(self._h, C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+
+    def thermo(self, T, p, Y, cp=None, h=None):
+        n = T.numel()
+        cp = torch.empty_like(T) if cp is None else cp
+        h = torch.empty_like(T) if h is None else h
+        self._sync_stream()
+        _check(lib().crf_thermo(self._h, _dev(T, (n,)), _dev(p), _dev(Y, (self.Ns, n)), n,
+                                _dev(cp, (n,)), _dev(h, (n,))))
+        return cp, h
+
+    def thermo_species(self, T):
+        n = T.numel()
+        out = [torch.empty((self.Ns, n), dtype=torch.float64, device=T.device) for _ in range(3)]
+        self._sync_stream()
+        _check(lib().crf_thermo_species(self._h, _dev(T, (n,)), n, *[_dev(o) for o in out]))
+        return tuple(out)
+
+    def production_rates(self, T, p, Y, omega=None, qdot=None):
+        n = T.numel()
+        omega = torch.empty_like(Y) if omega is None else omega
+        qdot = torch.empty_like(T) if qdot is None else qdot
+        self._sync_stream()
+        _check(lib().crf_production_rates(self._h, _dev(T, (n,)), _dev(p, (n,)), _dev(Y, (self.Ns, n)), n,
+                                          _dev(omega, (self.Ns, n)), _dev(qdot, (n,))))
+        return omega, qdot
+
+    def mix_transport(self, T, p, Y, mu=None, lam=None, rhoD=None):
+        n = T.numel()
+        mu = torch.empty_like(T) if mu is None else mu
+        lam = torch.empty_like(T) if lam is None else lam
+        rhoD = torch.empty_like(Y) if rhoD is None else rhoD
+        self._sync_stream()
+        _check(lib().crf_mix_transport(self._h, _dev(T, (n,)), _dev(p), _dev(Y, (self.Ns, n)), n,
+                                       _dev(mu, (n,)), _dev(lam, (n,)), _dev(rhoD, (self.Ns, n))))
+        return mu, lam, rhoD
+
+    def step_host(self, T, p, Y, out: dict | None = None) -> dict:
+        """Whole path with HOST tensors (pinned for full bandwidth); returns host tensors."""
+        n = T.numel()
+        if out is None:
+            mk = lambda *s: torch.empty(s, dtype=torch.float64)  # noqa: E731
+            out = dict(cp=mk(n), h=mk(n), omega=mk(self.Ns, n), qdot=mk(n), mu=mk(n), lam=mk(n),
+                       rhoD=mk(self.Ns, n))
+        _check(lib().crf_step_host(
+            self._h, _host(T, (n,)), _host(p, (n,)), _host(Y, (self.Ns, n)), n,
+            _host(out["cp"], (n,)), _host(out["h"], (n,)), _host(out["omega"], (self.Ns, n)),
+            _host(out["qdot"], (n,)), _host(out["mu"], (n,)), _host(out["lam"], (n,)),
+            _host(out["rhoD"], (self.Ns, n))))
+        return out

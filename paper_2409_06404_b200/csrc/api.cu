@@ -1,0 +1,330 @@
+// api.cu -- the C ABI of libcrf.so (include/crf.h): mechanism construction (host re-layout of the
+// packed tables + upload), argument checks, dispatch to the kernel launchers, the host-buffer
+// pipeline crf_step_host and the FP64 probe.
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/crf.h"
+#include "crf_internal.h"
+#include "launch.h"
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<int64_t> g_launches{0};
+
+int fail(int code, const std::string &msg)
+{
+    g_err = msg;
+    return code;
+}
+int fail_cuda(cudaError_t e, const char *where)
+{
+    return fail(CRF_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+// Host-side builder of the single device block that holds every table.
+struct BlockBuilder {
+    std::vector<unsigned char> bytes;
+    template <class T>
+    size_t add(const std::vector<T> &v)
+    {
+        size_t off = (bytes.size() + 255) & ~size_t(255);
+        bytes.resize(off + std::max<size_t>(v.size(), 1) * sizeof(T));
+        if (!v.empty()) std::memcpy(bytes.data() + off, v.data(), v.size() * sizeof(T));
+        return off;
+    }
+};
+
+constexpr int kSlots = 3;          // pipeline depth of crf_step_host
+constexpr int64_t kChunk = 65536;  // points per chunk
+
+}  // namespace
+
+void crf_count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+struct crf_mech {
+    DevTables dev{};
+    void *block = nullptr;
+    cudaStream_t stream = nullptr;
+    // crf_step_host resources (lazy)
+    cudaStream_t pipe_stream[kSlots] = {nullptr, nullptr, nullptr};
+    double *pipe_buf[kSlots] = {nullptr, nullptr, nullptr};
+    int64_t pipe_chunk = 0;
+};
+
+extern "C" {
+
+const char *crf_last_error(void) { return g_err.c_str(); }
+int64_t crf_launch_count(void) { return g_launches.load(); }
+
+int crf_mech_create(const crf_tables *t, crf_mech **out)
+{
+    if (!t || !out) return fail(CRF_EINVAL, "crf_mech_create: null argument");
+    if (t->version != CRF_TABLES_VERSION) return fail(CRF_EINVAL, "crf_mech_create: tables version mismatch");
+    const int Ns = t->Ns, Nr = t->Nr, N3 = t->N3, Nt = t->Nt;
+    if (Ns < 1 || Nr < 0 || N3 < 0 || Nt < 0 || N3 + Nt > Nr) return fail(CRF_EINVAL, "crf_mech_create: bad counts");
+    if (Ns > 220) return fail(CRF_EUNSUPPORTED, "crf_mech_create: more than 220 species");
+    if (!(t->p_ref > 0.0)) return fail(CRF_EINVAL, "crf_mech_create: p_ref must be positive");
+    const void *need[] = {t->W, t->Tmid, t->nasa_lo, t->nasa_hi, t->mu_c, t->lam_c, t->D_c};
+    for (const void *q : need)
+        if (!q) return fail(CRF_EINVAL, "crf_mech_create: null table");
+    if (Nr > 0 && (!t->lnA || !t->beta || !t->Ea_R || !t->reac || !t->prod))
+        return fail(CRF_EINVAL, "crf_mech_create: null reaction table");
+    if (N3 + Nt > 0 && (!t->eff_ptr || !t->eff_idx || !t->eff_val))
+        return fail(CRF_EINVAL, "crf_mech_create: null efficiency table");
+    if (Nt > 0 && (!t->lnA0 || !t->beta0 || !t->Ea0_R || !t->alpha || !t->T3 || !t->T1 || !t->T2))
+        return fail(CRF_EINVAL, "crf_mech_create: null falloff table");
+    for (int k = 0; k < Ns; ++k)
+        if (!(t->W[k] > 0.0)) return fail(CRF_EINVAL, "crf_mech_create: molar masses must be positive");
+
+    // ---- derived host tables ----
+    std::vector<double> W(t->W, t->W + Ns), rW(Ns), Tmid(t->Tmid, t->Tmid + Ns), wq(Ns);
+    for (int k = 0; k < Ns; ++k) {
+        rW[k] = 1.0 / W[k];
+        wq[k] = 1.0 / std::sqrt(std::sqrt(W[k]));
+    }
+    std::vector<double> cpc(2 * 5 * Ns), hc(2 * 6 * Ns), gc(2 * 7 * Ns), sc(2 * 6 * Ns);
+    for (int rg = 0; rg < 2; ++rg) {
+        const double *a = rg == 0 ? t->nasa_lo : t->nasa_hi;  // [7][Ns]
+        for (int k = 0; k < Ns; ++k) {
+            const double a1 = a[0 * Ns + k], a2 = a[1 * Ns + k], a3 = a[2 * Ns + k], a4 = a[3 * Ns + k],
+                         a5 = a[4 * Ns + k], a6 = a[5 * Ns + k], a7 = a[6 * Ns + k];
+            double *c = cpc.data() + rg * 5 * Ns + k;
+            c[0] = a1, c[Ns] = a2, c[2 * Ns] = a3, c[3 * Ns] = a4, c[4 * Ns] = a5;
+            double *h = hc.data() + rg * 6 * Ns + k;
+            h[0] = a1, h[Ns] = a2 / 2.0, h[2 * Ns] = a3 / 3.0, h[3 * Ns] = a4 / 4.0, h[4 * Ns] = a5 / 5.0,
+            h[5 * Ns] = a6;
+            double *s = sc.data() + rg * 6 * Ns + k;
+            s[0] = a1, s[Ns] = a2, s[2 * Ns] = a3 / 2.0, s[3 * Ns] = a4 / 3.0, s[4 * Ns] = a5 / 4.0, s[5 * Ns] = a7;
+            double *g = gc.data() + rg * 7 * Ns + k;
+            g[0] = a1, g[Ns] = -a2 / 2.0, g[2 * Ns] = -a3 / 6.0, g[3 * Ns] = -a4 / 12.0, g[4 * Ns] = -a5 / 20.0,
+            g[5 * Ns] = a6, g[6 * Ns] = -a7;
+        }
+    }
+    std::vector<double> lnA(t->lnA, t->lnA + Nr), beta(t->beta, t->beta + Nr), Ea_R(t->Ea_R, t->Ea_R + Nr), dnu(Nr);
+    std::vector<int16_t> reac(t->reac, t->reac + (size_t)kSlots * Nr), prod(t->prod, t->prod + (size_t)kSlots * Nr);
+    for (int r = 0; r < Nr; ++r) {
+        int nf = 0, nb = 0;
+        for (int s = 0; s < kSlots; ++s) {
+            const int a = reac[(size_t)s * Nr + r], b = prod[(size_t)s * Nr + r];
+            if (a >= Ns || b >= Ns || a < -1 || b < -1)
+                return fail(CRF_EINVAL, "crf_mech_create: species index out of range");
+            nf += a >= 0;
+            nb += b >= 0;
+        }
+        if (nf == 0 || nb == 0) return fail(CRF_EINVAL, "crf_mech_create: reaction without reactant or product");
+        dnu[r] = double(nb - nf);
+    }
+    const int nM = N3 + Nt;
+    std::vector<int32_t> eff_ptr(nM + 1, 0);
+    std::vector<int16_t> eff_idx;
+    std::vector<double> eff_val;
+    if (nM > 0) {
+        eff_ptr.assign(t->eff_ptr, t->eff_ptr + nM + 1);
+        if (eff_ptr[0] != 0) return fail(CRF_EINVAL, "crf_mech_create: eff_ptr[0] must be 0");
+        for (int r = 0; r < nM; ++r)
+            if (eff_ptr[r + 1] < eff_ptr[r]) return fail(CRF_EINVAL, "crf_mech_create: eff_ptr not monotone");
+        eff_idx.assign(t->eff_idx, t->eff_idx + eff_ptr[nM]);
+        eff_val.assign(t->eff_val, t->eff_val + eff_ptr[nM]);
+        for (int16_t k : eff_idx)
+            if (k < 0 || k >= Ns) return fail(CRF_EINVAL, "crf_mech_create: efficiency species out of range");
+    }
+    std::vector<double> lnA0, beta0, Ea0_R, alpha, rT3, rT1, T2;
+    if (Nt > 0) {
+        lnA0.assign(t->lnA0, t->lnA0 + Nt);
+        beta0.assign(t->beta0, t->beta0 + Nt);
+        Ea0_R.assign(t->Ea0_R, t->Ea0_R + Nt);
+        alpha.assign(t->alpha, t->alpha + Nt);
+        T2.assign(t->T2, t->T2 + Nt);
+        rT3.resize(Nt);
+        rT1.resize(Nt);
+        for (int i = 0; i < Nt; ++i) {
+            rT3[i] = 1.0 / t->T3[i];
+            rT1[i] = 1.0 / t->T1[i];
+        }
+    }
+    const int npair = Ns * (Ns + 1) / 2;
+    std::vector<double> mu_c(t->mu_c, t->mu_c + 4 * Ns), lam_c(t->lam_c, t->lam_c + 4 * Ns), nDc(4 * (size_t)npair),
+        wilke(Ns * (size_t)Ns);
+    for (int q = 0; q < npair; ++q)
+        for (int c = 0; c < 4; ++c) nDc[4 * (size_t)q + c] = -t->D_c[(size_t)c * npair + q];
+    for (int k = 0; k < Ns; ++k)
+        for (int j = 0; j < Ns; ++j) wilke[(size_t)k * Ns + j] = 1.0 / std::sqrt(8.0 * (1.0 + W[k] / W[j]));
+
+    // ---- one device block ----
+    BlockBuilder b;
+    const size_t oW = b.add(W), orW = b.add(rW), oTm = b.add(Tmid), ocp = b.add(cpc), ohc = b.add(hc), ogc = b.add(gc),
+                 osc = b.add(sc), olnA = b.add(lnA), obeta = b.add(beta), oEa = b.add(Ea_R), odnu = b.add(dnu),
+                 oreac = b.add(reac), oprod = b.add(prod), oep = b.add(eff_ptr), oei = b.add(eff_idx),
+                 oev = b.add(eff_val), olnA0 = b.add(lnA0), ob0 = b.add(beta0), oE0 = b.add(Ea0_R), oal = b.add(alpha),
+                 orT3 = b.add(rT3), orT1 = b.add(rT1), oT2 = b.add(T2), omu = b.add(mu_c), olam = b.add(lam_c),
+                 onD = b.add(nDc), owk = b.add(wilke), owq = b.add(wq);
+    crf_mech *mech = new (std::nothrow) crf_mech;
+    if (!mech) return fail(CRF_ECUDA, "crf_mech_create: out of host memory");
+    cudaError_t e = cudaMalloc(&mech->block, b.bytes.size());
+    if (e != cudaSuccess) {
+        delete mech;
+        return fail_cuda(e, "crf_mech_create: cudaMalloc");
+    }
+    e = cudaMemcpy(mech->block, b.bytes.data(), b.bytes.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaFree(mech->block);
+        delete mech;
+        return fail_cuda(e, "crf_mech_create: cudaMemcpy");
+    }
+    const unsigned char *base = static_cast<const unsigned char *>(mech->block);
+    auto D = [&](size_t off) { return reinterpret_cast<const double *>(base + off); };
+    DevTables &d = mech->dev;
+    d.Ns = Ns, d.Nr = Nr, d.Ne = Nr - N3 - Nt, d.N3 = N3, d.Nt = Nt, d.npair = npair, d.p_ref = t->p_ref;
+    d.W = D(oW), d.rW = D(orW), d.Tmid = D(oTm), d.cpc = D(ocp), d.hc = D(ohc), d.gc = D(ogc), d.sc = D(osc);
+    d.lnA = D(olnA), d.beta = D(obeta), d.Ea_R = D(oEa), d.dnu = D(odnu);
+    d.reac = reinterpret_cast<const int16_t *>(base + oreac);
+    d.prod = reinterpret_cast<const int16_t *>(base + oprod);
+    d.eff_ptr = reinterpret_cast<const int32_t *>(base + oep);
+    d.eff_idx = reinterpret_cast<const int16_t *>(base + oei);
+    d.eff_val = D(oev);
+    d.lnA0 = D(olnA0), d.beta0 = D(ob0), d.Ea0_R = D(oE0), d.alpha = D(oal), d.rT3 = D(orT3), d.rT1 = D(orT1),
+    d.T2 = D(oT2);
+    d.mu_c = D(omu), d.lam_c = D(olam), d.nDc = D(onD), d.wilke_c = D(owk), d.wq = D(owq);
+    *out = mech;
+    return CRF_OK;
+}
+
+void crf_mech_destroy(crf_mech *mech)
+{
+    if (!mech) return;
+    for (int s = 0; s < kSlots; ++s) {
+        if (mech->pipe_buf[s]) cudaFree(mech->pipe_buf[s]);
+        if (mech->pipe_stream[s]) cudaStreamDestroy(mech->pipe_stream[s]);
+    }
+    if (mech->block) cudaFree(mech->block);
+    delete mech;
+}
+
+int crf_mech_set_stream(crf_mech *mech, void *cuda_stream)
+{
+    if (!mech) return fail(CRF_EINVAL, "crf_mech_set_stream: null mechanism");
+    mech->stream = static_cast<cudaStream_t>(cuda_stream);
+    return CRF_OK;
+}
+int crf_mech_num_species(const crf_mech *mech) { return mech ? mech->dev.Ns : CRF_EINVAL; }
+int crf_mech_num_reactions(const crf_mech *mech) { return mech ? mech->dev.Nr : CRF_EINVAL; }
+
+#define CRF_CHECK_COMMON(name)                                                  \
+    if (!mech) return fail(CRF_EINVAL, name ": null mechanism");                \
+    if (n < 0) return fail(CRF_EINVAL, name ": negative n");                    \
+    if (n == 0) return CRF_OK;                                                  \
+    if (n > (int64_t)2147483647 * 32) return fail(CRF_EINVAL, name ": n too large");
+
+int crf_thermo(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *cp,
+               double *h)
+{
+    CRF_CHECK_COMMON("crf_thermo")
+    if (!T || !Y || !cp || !h) return fail(CRF_EINVAL, "crf_thermo: null pointer");
+    if (misaligned(T) || misaligned(Y) || misaligned(cp) || misaligned(h) || misaligned(p))
+        return fail(CRF_EINVAL, "crf_thermo: pointers must be 16-byte aligned");
+    cudaError_t e = launch_thermo(mech->dev, T, Y, n, cp, h, mech->stream);
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_thermo");
+}
+
+int crf_thermo_species(const crf_mech *mech, const double *T, int64_t n, double *cpk, double *hk, double *sk)
+{
+    CRF_CHECK_COMMON("crf_thermo_species")
+    if (!T) return fail(CRF_EINVAL, "crf_thermo_species: null pointer");
+    if (misaligned(T) || misaligned(cpk) || misaligned(hk) || misaligned(sk))
+        return fail(CRF_EINVAL, "crf_thermo_species: pointers must be 16-byte aligned");
+    cudaError_t e = launch_thermo_species(mech->dev, T, n, cpk, hk, sk, mech->stream);
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_thermo_species");
+}
+
+int crf_production_rates(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
+                         double *omega, double *qdot)
+{
+    CRF_CHECK_COMMON("crf_production_rates")
+    if (!T || !p || !Y || !omega || !qdot) return fail(CRF_EINVAL, "crf_production_rates: null pointer");
+    if (misaligned(T) || misaligned(p) || misaligned(Y) || misaligned(omega) || misaligned(qdot))
+        return fail(CRF_EINVAL, "crf_production_rates: pointers must be 16-byte aligned");
+    cudaError_t e = launch_rates(mech->dev, T, p, Y, n, omega, qdot, mech->stream);
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_production_rates");
+}
+
+int crf_mix_transport(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *mu,
+                      double *lambda, double *rhoD)
+{
+    CRF_CHECK_COMMON("crf_mix_transport")
+    if (!T || !Y || !mu || !lambda || !rhoD) return fail(CRF_EINVAL, "crf_mix_transport: null pointer");
+    if (misaligned(T) || misaligned(p) || misaligned(Y) || misaligned(mu) || misaligned(lambda) || misaligned(rhoD))
+        return fail(CRF_EINVAL, "crf_mix_transport: pointers must be 16-byte aligned");
+    cudaError_t e = launch_transport(mech->dev, T, p, Y, n, mu, lambda, rhoD, mech->stream);
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_mix_transport");
+}
+
+// Chunked host pipeline: slot s owns a stream and one device buffer holding, for a chunk of c points,
+// T, p, Y[Ns], cp, h, qdot, mu, lambda, omega[Ns], rhoD[Ns] (each row c doubles).
+int crf_step_host(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *cp, double *h,
+                  double *omega, double *qdot, double *mu, double *lambda, double *rhoD)
+{
+    CRF_CHECK_COMMON("crf_step_host")
+    if (!T || !p || !Y || !cp || !h || !omega || !qdot || !mu || !lambda || !rhoD)
+        return fail(CRF_EINVAL, "crf_step_host: null pointer");
+    const int Ns = mech->dev.Ns;
+    const int64_t chunk = kChunk;
+    const size_t rows = 7 + 3 * (size_t)Ns;
+    cudaError_t e;
+    if (mech->pipe_chunk != chunk) {
+        for (int s = 0; s < kSlots; ++s) {
+            if (!mech->pipe_stream[s]) {
+                e = cudaStreamCreateWithFlags(&mech->pipe_stream[s], cudaStreamNonBlocking);
+                if (e != cudaSuccess) return fail_cuda(e, "crf_step_host: stream");
+            }
+            if (mech->pipe_buf[s]) cudaFree(mech->pipe_buf[s]);
+            e = cudaMalloc(&mech->pipe_buf[s], rows * chunk * sizeof(double));
+            if (e != cudaSuccess) return fail_cuda(e, "crf_step_host: cudaMalloc");
+        }
+        mech->pipe_chunk = chunk;
+    }
+    int slot = 0;
+    for (int64_t off = 0; off < n; off += chunk, slot = (slot + 1) % kSlots) {
+        const int64_t c = std::min(chunk, n - off);
+        cudaStream_t st = mech->pipe_stream[slot];
+        double *b = mech->pipe_buf[slot];
+        double *dT = b, *dp = b + chunk, *dY = b + 2 * chunk, *dcp = dY + (size_t)Ns * chunk, *dh = dcp + chunk,
+               *dq = dh + chunk, *dmu = dq + chunk, *dlam = dmu + chunk, *dom = dlam + chunk,
+               *drD = dom + (size_t)Ns * chunk;
+        const size_t w = (size_t)c * sizeof(double);
+#define CRF_TRY(call)                                              \
+    if ((e = (call)) != cudaSuccess) return fail_cuda(e, "crf_step_host: " #call);
+        CRF_TRY(cudaMemcpyAsync(dT, T + off, w, cudaMemcpyHostToDevice, st))
+        CRF_TRY(cudaMemcpyAsync(dp, p + off, w, cudaMemcpyHostToDevice, st))
+        CRF_TRY(cudaMemcpy2DAsync(dY, w, Y + off, (size_t)n * sizeof(double), w, Ns, cudaMemcpyHostToDevice, st))
+        // kernels see a compact chunk: leading dimension c
+        CRF_TRY(launch_thermo(mech->dev, dT, dY, c, dcp, dh, st))
+        CRF_TRY(launch_rates(mech->dev, dT, dp, dY, c, dom, dq, st))
+        CRF_TRY(launch_transport(mech->dev, dT, dp, dY, c, dmu, dlam, drD, st))
+        CRF_TRY(cudaMemcpyAsync(cp + off, dcp, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpyAsync(h + off, dh, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpyAsync(qdot + off, dq, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpyAsync(mu + off, dmu, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpyAsync(lambda + off, dlam, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpy2DAsync(omega + off, (size_t)n * sizeof(double), dom, w, w, Ns, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpy2DAsync(rhoD + off, (size_t)n * sizeof(double), drD, w, w, Ns, cudaMemcpyDeviceToHost, st))
+    }
+    for (int s = 0; s < kSlots; ++s) CRF_TRY(cudaStreamSynchronize(mech->pipe_stream[s]))
+#undef CRF_TRY
+    return CRF_OK;
+}
+
+int crf_fp64_probe(int iters, double *inst_per_s)
+{
+    if (iters < 1 || !inst_per_s) return fail(CRF_EINVAL, "crf_fp64_probe: bad argument");
+    cudaError_t e = launch_fp64_probe(iters, inst_per_s);
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_fp64_probe");
+}
+
+}  // extern "C"
