@@ -1,0 +1,204 @@
+"""GPU parity tests proper: the CUDA path, called through the C ABI (ctypes binding), against
+the CPU oracle on the same seeded inputs.  Tolerances are BASELINE.json's (tests/parity.py).
+
+* element by element at sizes the oracle finishes in seconds, spanning several thread blocks
+  and a ragged (odd) tail, for the five mechanisms C1..C5 in both h_f modes of the generator;
+* at BASELINE.json's full sizes, in the launch configuration bench.py times, on sampled
+  points (the path is pointwise, so the oracle evaluates the sampled columns one by one);
+* edge cases: n = 0, n = 1, odd n, pure species (the D_kk guard), T exactly at T_mid,
+  misaligned and null pointers, a non-default stream.
+"""
+import ctypes as C
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2409_06404_b200 import workloads as wl
+from tests import parity
+from tests.helpers import P_REF, rxn, tiny_mech
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def binding():
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2409_06404_b200 import binding as b
+    b.lib()  # raises if libcrf.so is missing: there is no fallback
+    return b
+
+
+_cache = {}
+
+
+def _mech_pair(binding, oracle_mod, name, hf="uniform"):
+    key = (name, hf)
+    if key not in _cache:
+        desc = wl.make_mechanism(name, hf=hf)
+        _cache[key] = (desc, binding.Mechanism(desc), oracle_mod.Oracle(desc))
+    return _cache[key]
+
+
+SMALL_N = {"C1": 512, "C2": 2 * 1024 + 333, "C3": 3 * 1024 + 77, "C4": 1024 + 301, "C5": 512 + 129}
+
+
+@pytest.mark.parametrize("hf", ["uniform", "group"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+def test_elementwise_small(binding, oracle_mod, name, hf):
+    desc, gm, om = _mech_pair(binding, oracle_mod, name, hf)
+    n = SMALL_N[name]
+    st = wl.make_state(name, n=n, total=n)
+    e = parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), f"{name}/{hf} n={n}")
+    print(name, hf, {k: f"{v:.3g}" for k, v in e.items()})
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_full_size_sampled(binding, oracle_mod, name):
+    """Full BASELINE.json size, device-resident, same calls bench.py times; 384 sampled points
+    (always including the first and last point and a block boundary) checked against the oracle."""
+    desc, gm, om = _mech_pair(binding, oracle_mod, name)
+    n = wl.config_points(name)
+    st = wl.make_state(name)
+    gpu = parity.run_gpu(gm, st)
+    rng = np.random.default_rng(123)
+    idx = np.unique(np.concatenate(([0, 1, 127, 128, 255, 256, n - 2, n - 1], rng.integers(0, n, 376))))
+    sub = dict(T=st["T"][idx], p=st["p"][idx], Y=np.ascontiguousarray(st["Y"][:, idx]))
+    gsub = {k: (v[:, idx] if v.ndim == 2 else v[idx]) for k, v in gpu.items()}
+    parity.assert_parity(gsub, parity.run_oracle(om, sub), f"{name} full n={n}")
+    # properties that hold at any size, over the whole field
+    for key in ("cp", "mu", "lam", "rhoD"):
+        assert np.all(np.isfinite(gpu[key])) and np.all(gpu[key] > 0.0), key
+    assert np.all(np.isfinite(gpu["omega"])) and np.all(np.isfinite(gpu["qdot"])) and np.all(np.isfinite(gpu["h"]))
+    # mass conservation sum_k W_k omega_k = 0 within the rate tolerance scale of the sampled points
+    W = np.asarray(desc["W"])
+    ref = om.production_rates(**sub)
+    assert np.all(np.abs(W @ gsub["omega"]) <= 1e-10 * (W @ ref["S_omega"]) + 1e-30)
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 31, 33, 127, 129, 255, 257])
+def test_ragged_sizes(binding, oracle_mod, n):
+    desc, gm, om = _mech_pair(binding, oracle_mod, "C3")
+    st = wl.make_state("C3", n=n, total=max(n, 1))
+    if n == 0:
+        d = parity.to_dev(st)
+        gm.thermo(d["T"], d["p"], d["Y"])
+        gm.production_rates(d["T"], d["p"], d["Y"])
+        gm.mix_transport(d["T"], d["p"], d["Y"])
+        torch.cuda.synchronize()
+        return
+    parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), f"C3 n={n}")
+
+
+def test_outputs_do_not_spill_past_n(binding, oracle_mod):
+    """Rows of the species-major outputs are written for exactly n points (guard cells untouched)."""
+    desc, gm, om = _mech_pair(binding, oracle_mod, "C1")
+    n, pad = 130, 6
+    st = wl.make_state("C1", n=n)
+    d = parity.to_dev(st)
+    Ns = gm.Ns
+    big = torch.full((Ns * n + pad,), -777.0, dtype=torch.float64, device="cuda")
+    big2 = torch.full((Ns * n + pad,), -777.0, dtype=torch.float64, device="cuda")
+    qd = torch.full((n + pad,), -777.0, dtype=torch.float64, device="cuda")
+    gm.production_rates(d["T"], d["p"], d["Y"], omega=big[: Ns * n].view(Ns, n), qdot=qd[:n])
+    gm.mix_transport(d["T"], d["p"], d["Y"], rhoD=big2[: Ns * n].view(Ns, n))
+    torch.cuda.synchronize()
+    assert torch.all(big[Ns * n:] == -777.0) and torch.all(big2[Ns * n:] == -777.0) and torch.all(qd[n:] == -777.0)
+    assert not torch.any(big[: Ns * n] == -777.0)
+
+
+def test_pure_species_and_tmid(binding, oracle_mod):
+    """Degenerate cases: each species pure (sum_{j!=k} X_j/D_jk == 0 -> rho D_kk), Y with exact
+    zeros, and T exactly at (and one ulp around) each species' T_mid."""
+    desc, gm, om = _mech_pair(binding, oracle_mod, "C3")
+    Ns = gm.Ns
+    tm = np.asarray(desc["nasa_Tmid"])
+    Tm = np.concatenate((tm, np.nextafter(tm, 0.0), np.nextafter(tm, 1e9)))
+    n = Ns + Tm.size
+    Y = np.zeros((Ns, n))
+    Y[np.arange(Ns), np.arange(Ns)] = 1.0
+    rng = np.random.default_rng(3)
+    Yr = rng.dirichlet(np.full(Ns, 0.5), size=Tm.size).T
+    Yr[rng.random(Yr.shape) < 0.3] = 0.0
+    Yr[0] += 1e-3
+    Y[:, Ns:] = Yr / Yr.sum(axis=0)
+    T = np.concatenate((rng.uniform(300, 2500, Ns), Tm))
+    st = dict(T=T, p=np.full(n, 2.5e5), Y=np.ascontiguousarray(Y))
+    gpu, ref = parity.run_gpu(gm, st), parity.run_oracle(om, st)
+    parity.assert_parity(gpu, ref, "pure species / T_mid")
+    # the guard really was hit: pure-species rows equal rho D_kk in the oracle
+    assert np.all(ref["rhoD"][np.arange(Ns), np.arange(Ns)] > 0)
+
+
+def test_hand_built_mechanism(binding, oracle_mod):
+    """A three-slot reaction (2A + B <=> C + D + E is outside the generator's forms), a reaction with
+    coefficient 2 and a falloff reaction without listed efficiencies."""
+    W = [2.0, 32.0, 18.0, 17.0, 1.0, 28.0]
+    troe = dict(A0=1e17, beta0=-0.5, Ea0=5.0, alpha=0.6, T3=100.0, T1=2000.0, T2=5000.0)
+    rx = [rxn([(0, 2), (1, 1)], [(2, 1), (3, 1), (4, 1)], A=1e11, beta=0.3, Ea=20.0),
+          rxn([(3, 2)], [(2, 1), (4, 2)], A=1e9, beta=1.0, Ea=40.0),
+          rxn([(3, 1), (4, 1)], [(2, 1)], A=1e13, beta=-0.2, Ea=3.0, type="falloff", eff={}, troe=troe),
+          rxn([(4, 2)], [(0, 1)], A=1e16, beta=-1.0, Ea=0.0, type="three_body", eff={0: 2.5, 2: 12.0})]
+    desc = tiny_mech(W, rx)
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    rng = np.random.default_rng(0)
+    n = 257
+    Y = rng.dirichlet(np.ones(6), size=n).T
+    st = dict(T=rng.uniform(300, 2500, n), p=rng.uniform(1e4, 1e7, n), Y=np.ascontiguousarray(Y))
+    parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), "hand-built")
+
+
+def test_species_thermo(binding, oracle_mod):
+    desc, gm, om = _mech_pair(binding, oracle_mod, "C4")
+    T = np.random.default_rng(1).uniform(250, 3200, 1001)
+    cpk, hk, sk = (t.cpu().numpy() for t in gm.thermo_species(torch.from_numpy(T).cuda()))
+    ref = om.thermo_species(T)
+    np.testing.assert_allclose(cpk, ref["cpk"], rtol=1e-12)
+    np.testing.assert_allclose(sk, ref["sk"], rtol=1e-12)
+    assert np.all(np.abs(hk - ref["hk"]) <= 1e-12 * np.maximum(np.abs(ref["hk"]), 1e-3 * ref["cpk"] * T))
+
+
+def test_stream_and_errors(binding, oracle_mod):
+    desc, gm, om = _mech_pair(binding, oracle_mod, "C1")
+    st = wl.make_state("C1", n=512)
+    ref = parity.run_oracle(om, st)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        gpu = parity.run_gpu(gm, st)
+    parity.assert_parity(gpu, ref, "side stream")
+    d = parity.to_dev(st)
+    L = binding.lib()
+    n = 512
+    out = torch.empty(9 * n + 2, dtype=torch.float64, device="cuda")
+    q = torch.empty(n, dtype=torch.float64, device="cuda")
+    args = (gm._h, d["T"].data_ptr(), d["p"].data_ptr(), d["Y"].data_ptr())
+    assert L.crf_production_rates(*args, n, out.data_ptr() + 8, q.data_ptr()) == -1  # misaligned
+    assert b"aligned" in L.crf_last_error()
+    assert L.crf_production_rates(*args, n, None, q.data_ptr()) == -1                # null
+    assert L.crf_production_rates(*args, -5, out.data_ptr(), q.data_ptr()) == -1     # negative n
+    assert L.crf_mix_transport(None, d["T"].data_ptr(), d["p"].data_ptr(), d["Y"].data_ptr(), n,
+                               q.data_ptr(), q.data_ptr(), out.data_ptr()) == -1
+    with pytest.raises(binding.CrfError):
+        gm.thermo(d["T"].float(), d["p"], d["Y"])
+
+
+def test_step_host_matches_device_calls(binding, oracle_mod):
+    """crf_step_host (host buffers, chunked pipeline) gives bit-identical results to the device calls
+    on a size that spans several chunks with a ragged last chunk."""
+    desc, gm, om = _mech_pair(binding, oracle_mod, "C3")
+    n = 2 * 65536 + 12345
+    st = wl.make_state("C3", n=n)
+    gpu = parity.run_gpu(gm, st)
+    host = {k: torch.from_numpy(v).pin_memory() for k, v in st.items()}
+    out = gm.step_host(host["T"], host["p"], host["Y"])
+    for key in ("cp", "h", "omega", "qdot", "mu", "lam", "rhoD"):
+        np.testing.assert_array_equal(out[key].numpy(), gpu[key], err_msg=key)
+    idx = np.random.default_rng(5).integers(0, n, 256)
+    sub = dict(T=st["T"][idx], p=st["p"][idx], Y=np.ascontiguousarray(st["Y"][:, idx]))
+    hsub = {k: (v.numpy()[:, idx] if v.ndim == 2 else v.numpy()[idx]) for k, v in out.items()}
+    parity.assert_parity(hsub, parity.run_oracle(om, sub), "step_host")
+
+
+def test_fp64_probe(binding):
+    r = binding.fp64_probe(2048)
+    assert 1e12 < r < 4e13, r  # B200: 148 SM x 64 lanes x ~1.9 GHz = 1.8e13 FP64 instr/s nominal
