@@ -10,6 +10,7 @@
 
 #include "../../include/crf.h"
 #include "crf_internal.h"
+#include "host_plan.h"
 #include "launch.h"
 
 namespace {
@@ -27,19 +28,6 @@ int fail_cuda(cudaError_t e, const char *where)
     return fail(CRF_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
 }
 bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
-
-// Host-side builder of the single device block that holds every table.
-struct BlockBuilder {
-    std::vector<unsigned char> bytes;
-    template <class T>
-    size_t add(const std::vector<T> &v)
-    {
-        size_t off = (bytes.size() + 255) & ~size_t(255);
-        bytes.resize(off + std::max<size_t>(v.size(), 1) * sizeof(T));
-        if (!v.empty()) std::memcpy(bytes.data() + off, v.data(), v.size() * sizeof(T));
-        return off;
-    }
-};
 
 constexpr int kSlots = 3;          // pipeline depth of crf_step_host
 constexpr int64_t kChunk = 65536;  // points per chunk
@@ -165,6 +153,8 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
                  oev = b.add(eff_val), olnA0 = b.add(lnA0), ob0 = b.add(beta0), oE0 = b.add(Ea0_R), oal = b.add(alpha),
                  orT3 = b.add(rT3), orT1 = b.add(rT1), oT2 = b.add(T2), omu = b.add(mu_c), olam = b.add(lam_c),
                  onD = b.add(nDc), owk = b.add(wilke), owq = b.add(wq);
+    const TransportPlanOffsets tpo = build_transport_plan(t, b);
+    const RatesPlanOffsets rpo = build_rates_plan(t, b);
     crf_mech *mech = new (std::nothrow) crf_mech;
     if (!mech) return fail(CRF_ECUDA, "crf_mech_create: out of host memory");
     cudaError_t e = cudaMalloc(&mech->block, b.bytes.size());
@@ -192,6 +182,18 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
     d.lnA0 = D(olnA0), d.beta0 = D(ob0), d.Ea0_R = D(oE0), d.alpha = D(oal), d.rT3 = D(orT3), d.rT1 = D(orT1),
     d.T2 = D(oT2);
     d.mu_c = D(omu), d.lam_c = D(olam), d.nDc = D(onD), d.wilke_c = D(owk), d.wq = D(owq);
+    TransportPlan &tp = d.tp;
+    tp.W = tpo.W, tp.NsP = tpo.NsP, tp.nb = tpo.nb, tp.n_rounds = tpo.n_rounds;
+    tp.sched = reinterpret_cast<const int2 *>(base + tpo.sched);
+    tp.pair_coef = D(tpo.pair_coef), tp.wilke_cP = D(tpo.wilke_cP), tp.sp = D(tpo.sp), tp.Ddiag = D(tpo.Ddiag);
+    RatesPlan &rp = d.rp;
+    rp.W = rpo.W, rp.Rc = rpo.Rc, rp.n_chunks = rpo.n_chunks;
+    rp.chunk = reinterpret_cast<const int4 *>(base + rpo.chunk);
+    rp.rc = D(rpo.rc);
+    rp.rs = reinterpret_cast<const int4 *>(base + rpo.rs);
+    rp.inc_ptr = reinterpret_cast<const int *>(base + rpo.inc_ptr);
+    rp.inc = reinterpret_cast<const double2 *>(base + rpo.inc);
+    rp.troe = D(rpo.troe), rp.gco = D(rpo.gco), rp.hco = D(rpo.hco);
     *out = mech;
     return CRF_OK;
 }

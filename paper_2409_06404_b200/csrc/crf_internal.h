@@ -6,6 +6,38 @@
 
 #define CRF_R_GAS 8314.46261815324  // J/(kmol K)
 
+// Plan of the tiled crf_mix_transport kernel (transport_tiled.cu): species padded to blocks of 8,
+// the pair triangle cut into 8x8 tiles, tiles dealt to the W warps that share 32 points in rounds
+// whose tiles touch disjoint species blocks (so the warps update disjoint rows of S).
+struct TransportPlan {
+    int W;         // warps per block (1, 2 or 4); 0 = no plan (generic kernel)
+    int NsP, nb;   // padded species count (multiple of 8) and number of 8-blocks
+    int n_rounds;
+    const int2 *sched;        // [n_rounds][W]: x = kind | jb << 8 | kb << 16 (kind 0 idle, 1 off-diagonal,
+                              //   2 diagonal), y = offset of the tile's coefficients in pair_coef (doubles)
+    const double *pair_coef;  // schedule order; per pair (c0,c1,c2,c3) of -log2(e) * ln D_jk fit; 0 for padding
+    const double *wilke_cP;   // [NsP][NsP] c_kj = 1/sqrt(8 (1 + W_k/W_j)), 0 in padded rows/columns
+    const double *sp;         // [NsP][12]: 0-3 ln(mu_k)/2 cubic, 4-7 ln(lambda_k) cubic, 8 W^-1/4, 9 W^1/2,
+                              //   10 1/W (0 for padding), 11 unused
+    const double *Ddiag;      // [Ns][4] ln D_kk cubic (pure-species guard)
+};
+
+// Plan of the staged crf_production_rates kernel (rates_staged.cu).
+struct RatesPlan {
+    int W;        // warps per block; 0 = no plan
+    int Rc;       // reactions per chunk (q buffer rows)
+    int n_chunks;
+    const int4 *chunk;      // [n_chunks]: x = type (0 elementary, 1 third-body, 2 falloff), y = first reaction,
+                            //   z = count, w = first row of the third-body/falloff tables
+    const double *rc;       // [Nr][4]: log2(e) lnA, beta, -log2(e) Ea/R, dnu
+    const int4 *rs;         // [Nr][2]: byte offsets into the (C,g) state of reactants (3) and products (3); -1 = empty
+    const int *inc_ptr;     // [n_chunks][Ns+1] incidence lists of each chunk, species-major
+    const double2 *inc;     // entries: x = nu_kr (signed), y = bit pattern of the q-row byte offset
+    const double *troe;     // [Nt][8]: log2e lnA0, beta0, -log2e Ea0/R, alpha, -log2e/T3, -log2e/T1, -log2e T2, 0
+    const double *gco;      // [Ns][16]: g/(RT) Horner sets, low range 0-6, high range 8-14, 7 = Tmid, 15 = 1/W
+    const double *hco;      // [Ns][16]: h/(RT) sets, low 0-5, high 8-13
+};
+
 // Device-resident tables, re-laid-out by crf_mech_create from crf_tables.
 // All pointers are device pointers into one allocation owned by crf_mech.
 struct DevTables {
@@ -34,6 +66,8 @@ struct DevTables {
     const double *nDc;           // [npair][4]  NEGATED D_jk fit, pair-major: exp gives 1/D_jk(p_ref)
     const double *wilke_c;       // [Ns][Ns]    c_kj = 1/sqrt(8 (1 + W_k/W_j))
     const double *wq;            // [Ns]        W_k^(-1/4)
+    TransportPlan tp;
+    RatesPlan rp;
 };
 
 __device__ __forceinline__ int crf_pair_index(int j, int k, int ns)

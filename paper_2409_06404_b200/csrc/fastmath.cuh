@@ -1,0 +1,41 @@
+// fastmath.cuh -- the one transcendental the hot loops are made of: 2^y on the FP64 pipe.
+//
+// The pair loop of crf_mix_transport and the reaction loop of crf_production_rates spend
+// three quarters of their FP64 instructions in exp().  libdevice's exp() costs 14 DFMA + 1 DADD
+// and is accurate to < 1 ulp; the tolerances of this path (1e-12 relative for transport, 1e-10
+// of the gross rate for omega) allow a shorter evaluation:
+//
+//   y  = x * log2(e) is folded into the table coefficients on the host, so the kernels evaluate
+//        2^y directly;
+//   k  = rint(y) by the magic-number add, f = y - k in [-1/2, 1/2]              (3 DADD)
+//   2^f = degree-9 polynomial, Chebyshev-node interpolant, relative error 1.9e-14  (9 DFMA)
+//   2^k by an integer add into the exponent field                               (1 IADD)
+//
+// Domain: |y| < 1000 (no overflow/underflow/NaN handling).  y = -inf (an exact zero
+// concentration in log space) is not supported; callers that can see it use exp().
+#pragma once
+
+namespace crf {
+
+__device__ __forceinline__ double exp2_poly9(double y)
+{
+    const double magic = 6755399441055744.0;  // 1.5 * 2^52
+    const double t = __dadd_rn(y, magic);
+    const int k = __double2loint(t);
+    const double f = __dsub_rn(y, __dsub_rn(t, magic));
+    double p = 0x1.b6571de2f2351p-24;
+    p = fma(p, f, 0x1.63ef969a64d3cp-20);
+    p = fma(p, f, 0x1.ffcb76789860fp-17);
+    p = fma(p, f, 0x1.43088e257f341p-13);
+    p = fma(p, f, 0x1.5d87fe908f88ap-10);
+    p = fma(p, f, 0x1.3b2ab72b175eep-7);
+    p = fma(p, f, 0x1.c6b08d7044119p-5);
+    p = fma(p, f, 0x1.ebfbdff8149f2p-3);
+    p = fma(p, f, 0x1.62e42fefa39f7p-1);
+    p = fma(p, f, 0x1.000000000003dp+0);
+    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+constexpr double kLog2e = 1.4426950408889634074;
+
+}  // namespace crf
