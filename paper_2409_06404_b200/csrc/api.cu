@@ -155,6 +155,7 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
                  onD = b.add(nDc), owk = b.add(wilke), owq = b.add(wq);
     const TransportPlanOffsets tpo = build_transport_plan(t, b);
     const RatesPlanOffsets rpo = build_rates_plan(t, b);
+    const RatesSmemPlanOffsets rso = build_rates_smem_plan(t, b);
     crf_mech *mech = new (std::nothrow) crf_mech;
     if (!mech) return fail(CRF_ECUDA, "crf_mech_create: out of host memory");
     cudaError_t e = cudaMalloc(&mech->block, b.bytes.size());
@@ -194,6 +195,11 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
     rp.inc_ptr = reinterpret_cast<const int *>(base + rpo.inc_ptr);
     rp.inc = reinterpret_cast<const double2 *>(base + rpo.inc);
     rp.troe = D(rpo.troe), rp.gco = D(rpo.gco), rp.hco = D(rpo.hco);
+    RatesSmemPlan &rs = d.rs;
+    rs.W = rso.W, rs.PPL = rso.PPL, rs.Rc = rso.Rc, rs.n_chunks = rso.n_chunks, rs.stage_bytes = rso.stage_bytes;
+    rs.chunk = reinterpret_cast<const int4 *>(base + rso.chunk);
+    rs.stage = base + rso.stage;
+    rs.gco = D(rso.gco), rs.hco = D(rso.hco);
     *out = mech;
     return CRF_OK;
 }

@@ -38,6 +38,31 @@ struct RatesPlan {
     const double *hco;      // [Ns][16]: h/(RT) sets, low 0-5, high 8-13
 };
 
+// Plan of the shared-memory-staged crf_production_rates kernel (rates_smem.cu): the reactions are cut into
+// chunks of one kind; everything a chunk needs (reaction records, per-species incidence lists, third-body
+// lists, Troe sets) is one contiguous block of `stage` that the thread block copies into shared memory
+// with cp.async while it works on the previous chunk.  Layout of a chunk block (byte offsets from its start):
+//   [0, 48 count)            reaction records: f64 log2(e) lnA, f64 beta, f64 -log2(e) Ea/R, u32 x0, u32 x1,
+//                            u32 a0, a1, b0, b1 (byte offsets of the reactant/product rows in the state);
+//                            x0, x1 = third reactant/product rows (generic kinds) or offset/count of the
+//                            third-body list (kinds 1, 2)
+//   [48 count, +8 Ns)        per species (start, end) byte offsets of its incidence entries
+//   then (16-byte aligned)   Troe sets, 64 bytes per reaction (kind 2 only)
+//   then                     incidence entries {f64 nu, u32 byte offset of q_r, u32 0} and third-body
+//                            entries {f64 efficiency - 1, u32 state row offset, u32 0}
+struct RatesSmemPlan {
+    int W;            // warps sharing a point group; 0 = no plan
+    int PPL;          // points per lane (1 or 2)
+    int Rc;           // q buffer rows (max reactions per chunk)
+    int n_chunks;
+    int stage_bytes;  // largest chunk block, multiple of 16
+    const int4 *chunk;           // [n_chunks]: x = kind (0 elementary, 1 third body, 2 falloff) | generic << 2,
+                                 //   y = reactions, z = byte offset of the block in stage, w = block bytes
+    const unsigned char *stage;
+    const double *gco;  // [Ns][16]: log2(e) g/(RT) Horner sets, low range 0-6, high range 8-14, 7 = Tmid, 15 = 1/W
+    const double *hco;  // [Ns][16]: h/(RT) sets, low 0-5, high 8-13, 7 = Tmid
+};
+
 // Device-resident tables, re-laid-out by crf_mech_create from crf_tables.
 // All pointers are device pointers into one allocation owned by crf_mech.
 struct DevTables {
@@ -68,6 +93,7 @@ struct DevTables {
     const double *wq;            // [Ns]        W_k^(-1/4)
     TransportPlan tp;
     RatesPlan rp;
+    RatesSmemPlan rs;
 };
 
 __device__ __forceinline__ int crf_pair_index(int j, int k, int ns)

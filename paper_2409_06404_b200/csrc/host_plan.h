@@ -31,5 +31,11 @@ struct RatesPlanOffsets {
     size_t chunk = 0, rc = 0, rs = 0, inc_ptr = 0, inc = 0, troe = 0, gco = 0, hco = 0;
 };
 
+struct RatesSmemPlanOffsets {
+    int W = 0, PPL = 0, Rc = 0, n_chunks = 0, stage_bytes = 0;
+    size_t chunk = 0, stage = 0, gco = 0, hco = 0;
+};
+
 TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b);
 RatesPlanOffsets build_rates_plan(const crf_tables *t, BlockBuilder &b);
+RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b);

@@ -16,4 +16,6 @@ cudaError_t launch_transport_tiled(const DevTables &m, const double *T, const do
                                    double *lambda, double *rhoD, cudaStream_t st);
 cudaError_t launch_rates_staged(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                                 double *omega, double *qdot, cudaStream_t st);
+cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
+                              double *omega, double *qdot, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *inst_per_s);

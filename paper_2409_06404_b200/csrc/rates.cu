@@ -149,6 +149,7 @@ cudaError_t launch_b(const DevTables &m, const double *T, const double *p, const
 cudaError_t launch_rates(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                          double *omega, double *qdot, cudaStream_t st)
 {
+    if (m.rs.W > 0) return launch_rates_smem(m, T, p, Y, n, omega, qdot, st);
     if (m.rp.W > 0) return launch_rates_staged(m, T, p, Y, n, omega, qdot, st);
     const size_t per_thread = sizeof(double) * 2 * (size_t)m.Ns;
     const size_t budget = 100 * 1024;  // two blocks per SM

@@ -1,0 +1,417 @@
+// rates_smem.cu -- crf_production_rates, the kernel the library uses
+// whenever the mechanism admits its plan (plan_rates_smem.cu); rates_staged.cu / rates.cu are the fallbacks.
+//
+// Shape.  W warps share a group of 32 PPL grid points (lane = point, PPL points per lane), so every
+// mechanism coefficient is a warp-uniform shared-memory load.  Per point and species the block keeps
+// (C_k, d_k), d_k = (p_ref/RT) exp(-g_k/RT), in shared memory as [species][point] rows of double2.
+//
+//   k_f        = 2^(log2e lnA + log2e beta ln T - log2e Ea/(R T))                 one exponential per reaction
+//   1/K_c      = prod_reactants d / prod_products d                               (K_c = exp(-sum nu g/RT) (p_ref/RT)^dnu)
+//   q          = k_f [M] (prod_reactants C - (1/K_c) prod_products C)
+//
+// i.e. the second exponential of a reversible reaction is replaced by two multiplications and one
+// reciprocal (MUFU seed + one cubic Newton step); the exponentials of g_k are taken once per species and
+// point.  crf_mech_create admits this form only if numerator, denominator and quotient stay inside the
+// double range for every T in [250, 5000] K (plan_rates_smem.cu), otherwise rates_staged.cu runs.
+//
+// Reactions are cut into chunks of one kind (elementary | third body | Troe falloff; two or three
+// species per side).  A chunk's tables (48-byte reaction records, per-species incidence lists, third-body
+// lists, Troe sets) are one contiguous block that the thread block copies global -> shared with cp.async
+// while it works on the previous chunk (double buffer), so the reaction loop never waits on L2.
+//   reaction stage: the warps split the reactions of the chunk, q_r -> sQ[r][point];
+//   species stage:  the warps split the SPECIES; each owned species sums nu_kr q_r over its incidence list
+//                   into register accumulators that live for the whole kernel (omega never touches
+//                   shared memory).
+// Troe falloff is evaluated in base 2 (log2 F = log2 F_cent / (1 + f1^2)) with a branch-free logarithm.
+#include "crf_internal.h"
+#include "fastmath.cuh"
+#include "launch.h"
+
+namespace {
+
+__device__ __forceinline__ double exp2c(double y)
+{
+    // crf::exp2_poly9 with the exponent clamped from below: an underflowing rate constant becomes a
+    // negligible number instead of wrapping into the sign bit
+    const double magic = 6755399441055744.0;
+    const double t = __dadd_rn(y, magic);
+    const int k = max(__double2loint(t), -1000);
+    const double f = __dsub_rn(y, __dsub_rn(t, magic));
+    double p = 0x1.b6571de2f2351p-24;
+    p = fma(p, f, 0x1.63ef969a64d3cp-20);
+    p = fma(p, f, 0x1.ffcb76789860fp-17);
+    p = fma(p, f, 0x1.43088e257f341p-13);
+    p = fma(p, f, 0x1.5d87fe908f88ap-10);
+    p = fma(p, f, 0x1.3b2ab72b175eep-7);
+    p = fma(p, f, 0x1.c6b08d7044119p-5);
+    p = fma(p, f, 0x1.ebfbdff8149f2p-3);
+    p = fma(p, f, 0x1.62e42fefa39f7p-1);
+    p = fma(p, f, 0x1.000000000003dp+0);
+    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+// 1/x for normal x: MUFU.RCP64H seed (relative error < 2^-20) and one cubic Newton step
+__device__ __forceinline__ double rcp_fast(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    return fma(y, fma(e, e, e), y);
+}
+
+// log2(x) for normal x > 0, branch-free: x = 2^e m, m in [sqrt(1/2), sqrt(2)), ln m = 2 atanh((m-1)/(m+1))
+__device__ __forceinline__ double log2_fast(double x)
+{
+    int hi = __double2hiint(x);
+    const int e = (hi - 0x3fe6a09e) >> 20;
+    hi -= e << 20;
+    const double m = __hiloint2double(hi, __double2loint(x));
+    const double s = (m - 1.0) * rcp_fast(m + 1.0);
+    const double z = s * s;
+    double p = 1.0 / 17.0;
+    p = fma(p, z, 1.0 / 15.0);
+    p = fma(p, z, 1.0 / 13.0);
+    p = fma(p, z, 1.0 / 11.0);
+    p = fma(p, z, 1.0 / 9.0);
+    p = fma(p, z, 1.0 / 7.0);
+    p = fma(p, z, 1.0 / 5.0);
+    p = fma(p, z, 1.0 / 3.0);
+    p = fma(p, z, 1.0);
+    return fma(s * (2.0 * crf::kLog2e), p, (double)e);
+}
+
+template <int PPL>
+struct Ctx {
+    double T[PPL], L[PPL], rT[PPL];  // T, ln T, 1/T
+    double Csum[PPL];                // p/(R T)
+};
+
+__device__ __forceinline__ double2 lds2(const char *p) { return *reinterpret_cast<const double2 *>(p); }
+__device__ __forceinline__ uint4 ldsu4(const char *p) { return *reinterpret_cast<const uint4 *>(p); }
+
+// q of one reaction at the PPL points of this lane.  rec: the 48-byte record; tr: its Troe set (kind 2);
+// sL: the (C, d) state at this lane (row offsets come from the record; point u is 512 u bytes further).
+template <int KIND, bool GENERIC, int PPL>
+__device__ __forceinline__ void reaction_q(const char *blk, const char *rec, const char *tr, const char *sL,
+                                           const Ctx<PPL> &c, double (&q)[PPL])
+{
+    const double2 A = lds2(rec);        // log2e lnA, log2e beta
+    const double2 Ex = lds2(rec + 16);  // -log2e Ea/R, (x0, x1)
+    const uint4 S = ldsu4(rec + 32);    // a0, a1, b0, b1
+    const unsigned x0 = (unsigned)__double2loint(Ex.y), x1 = (unsigned)__double2hiint(Ex.y);
+    double M[PPL];
+    if (KIND != 0) {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) M[u] = c.Csum[u];
+        const char *e = blk + x0, *e1 = e + 16 * x1;
+        for (; e < e1; e += 16) {
+            const uint4 en = ldsu4(e);
+            const double coef = __hiloint2double((int)en.y, (int)en.x);
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) M[u] = fma(coef, lds2(sL + en.z + 512 * u).x, M[u]);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) {
+        const char *s = sL + 512 * u;
+        const double yinf = fma(A.y, c.L[u], fma(Ex.x, c.rT[u], A.x));  // log2 k_f (high-pressure limit)
+        const double2 a0 = lds2(s + S.x), a1 = lds2(s + S.y), b0 = lds2(s + S.z), b1 = lds2(s + S.w);
+        double Pf = a0.x * a1.x, Pr = b0.x * b1.x, num = a0.y * a1.y, den = b0.y * b1.y;
+        if (GENERIC) {
+            const double2 a2 = lds2(s + x0), b2 = lds2(s + x1);
+            Pf *= a2.x, Pr *= b2.x, num *= a2.y, den *= b2.y;
+        }
+        const double net = fma(-(num * rcp_fast(den)), Pr, Pf);  // prod C_reactants - prod C_products / K_c
+        if (KIND == 0) q[u] = exp2c(yinf) * net;
+        if (KIND == 1) q[u] = exp2c(yinf) * M[u] * net;
+        if (KIND == 2) {
+            // Troe falloff in base 2
+            const double2 t01 = lds2(tr), t23 = lds2(tr + 16), t45 = lds2(tr + 32), t67 = lds2(tr + 48);
+            const double y0 = fma(t01.y, c.L[u], fma(t23.x, c.rT[u], t01.x));
+            const double l2Pr = (y0 - yinf) + log2_fast(fmax(M[u], 1.0e-300));  // log2(k_0 [M] / k_inf)
+            const double al = t23.y;
+            const double Fc = fma(1.0 - al, exp2c(c.T[u] * t45.x),
+                                  fma(al, exp2c(c.T[u] * t45.y), exp2c(t67.x * c.rT[u])));
+            const double l2Fc = log2_fast(fmax(Fc, 1.0e-300));
+            const double l10_2 = 0.30102999566398119521;
+            const double lFc = l10_2 * l2Fc;
+            const double x = fma(l10_2, l2Pr, fma(-0.67, lFc, -0.4));  // log10 P_r + c
+            const double f1 = x * rcp_fast(fma(-0.14, x, fma(-1.27, lFc, 0.75)));
+            const double l2F = l2Fc * rcp_fast(fma(f1, f1, 1.0));
+            const double Pred = exp2c(l2Pr);
+            q[u] = exp2c(yinf + l2F) * (Pred * rcp_fast(1.0 + Pred)) * net;
+        }
+    }
+}
+
+template <int W, int PPL, int KIND, bool GENERIC>
+__device__ __forceinline__ void reaction_stage(const char *blk, int count, int o_troe, const char *sL, char *sQl,
+                                               int warp, const Ctx<PPL> &c)
+{
+    constexpr int NRX = PPL == 1 ? 2 : 1;  // independent reactions per trip (ILP = NRX * PPL chains)
+    int rl = warp;
+    for (; rl + (NRX - 1) * W < count; rl += NRX * W) {
+        double q[NRX][PPL];
+#pragma unroll
+        for (int v = 0; v < NRX; ++v)
+            reaction_q<KIND, GENERIC, PPL>(blk, blk + 48 * (rl + v * W), blk + o_troe + 64 * (rl + v * W), sL, c, q[v]);
+#pragma unroll
+        for (int v = 0; v < NRX; ++v)
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) *reinterpret_cast<double *>(sQl + (rl + v * W) * (256 * PPL) + 256 * u) = q[v][u];
+    }
+    if (NRX == 2 && rl < count) {
+        double q[PPL];
+        reaction_q<KIND, GENERIC, PPL>(blk, blk + 48 * rl, blk + o_troe + 64 * rl, sL, c, q);
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) *reinterpret_cast<double *>(sQl + rl * (256 * PPL) + 256 * u) = q[u];
+    }
+}
+
+__device__ __forceinline__ void stage_async(char *dst, const unsigned char *src, int bytes, int tid, int nthreads)
+{
+    for (int o = tid * 16; o < bytes; o += nthreads * 16) {
+        const unsigned d = (unsigned)__cvta_generic_to_shared(dst + o);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src + o) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void stage_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// the PPL points of a lane are adjacent: i0, i0 + 1 (one 128-bit access per row when n is even)
+template <int PPL>
+__device__ __forceinline__ void load_row(const double *__restrict__ row, int64_t i0, int64_t n, bool vec, double (&v)[PPL])
+{
+    if (PPL == 2 && vec && i0 + 1 < n) {
+        const double2 t = *reinterpret_cast<const double2 *>(row + i0);
+        v[0] = t.x, v[PPL - 1] = t.y;
+    } else {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) v[u] = row[min(i0 + u, n - 1)];
+    }
+}
+template <int PPL>
+__device__ __forceinline__ void store_row(double *__restrict__ row, int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
+{
+    if (PPL == 2 && vec && i0 + 1 < n) {
+        *reinterpret_cast<double2 *>(row + i0) = make_double2(v[0], v[PPL - 1]);
+    } else {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u)
+            if (i0 + u < n) row[i0 + u] = v[u];
+    }
+}
+
+template <int W, int PPL, int MAXOWN>
+__global__ void __launch_bounds__(32 * W, 16 / W)
+    rates_smem_kernel(DevTables m, const double *__restrict__ T, const double *__restrict__ p,
+                      const double *__restrict__ Y, int64_t n, double *__restrict__ omega, double *__restrict__ qdot)
+{
+    extern __shared__ double2 sm2[];
+    const RatesSmemPlan &rs = m.rs;
+    const int Ns = m.Ns;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    char *sCD = reinterpret_cast<char *>(sm2);                // [Ns + 1][PPL][32] (C_k, d_k); row Ns = (1, 1)
+    char *sQ = sCD + (size_t)(Ns + 1) * 512 * PPL;            // [Rc][PPL][32] q_r; also the reduction scratch
+    char *sStage = sQ + (size_t)rs.Rc * 256 * PPL;            // [2][stage_bytes]
+    char *sL = sCD + lane * 16;
+    char *sQl = sQ + lane * 8;
+    double *sred = reinterpret_cast<double *>(sQ);            // [W][PPL][32], valid outside the chunk loop
+
+    stage_async(sStage, rs.stage + __ldg(&rs.chunk[0].z), rs.stage_bytes, threadIdx.x, 32 * W);
+
+    const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * PPL;
+    const bool vec = (n & 1) == 0;
+    Ctx<PPL> c;
+    double pi[PPL], lc02[PPL];
+    load_row<PPL>(T, i0, n, vec, c.T);
+    load_row<PPL>(p, i0, n, vec, pi);
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) {
+        c.L[u] = log(c.T[u]);
+        c.rT[u] = 1.0 / c.T[u];
+        lc02[u] = crf::kLog2e * (log(m.p_ref / CRF_R_GAS) - c.L[u]);  // log2(p_ref/(R T))
+        c.Csum[u] = pi[u] * c.rT[u] * (1.0 / CRF_R_GAS);
+    }
+
+    // ---- a1, a2: Z_k = Y_k/W_k and d_k = 2^(log2(p_ref/RT) - log2e g_k/RT); warp w takes species w, w+W, ...
+    double invW[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) invW[u] = 0.0;
+    for (int k = warp; k < Ns; k += W) {
+        const double2 *g = reinterpret_cast<const double2 *>(rs.gco + 16 * (size_t)k);
+        const double2 l01 = __ldg(g), l23 = __ldg(g + 1), l45 = __ldg(g + 2), l6t = __ldg(g + 3);
+        const double2 h01 = __ldg(g + 4), h23 = __ldg(g + 5), h45 = __ldg(g + 6), h6w = __ldg(g + 7);
+        double y[PPL];
+        load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y);
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) {
+            const double Tu = c.T[u], oml = 1.0 - c.L[u];
+            double lo = fma(Tu, l45.x, l23.y);
+            lo = fma(Tu, lo, l23.x);
+            lo = fma(Tu, lo, l01.y);
+            lo = fma(Tu, lo, l6t.x);
+            lo = fma(l45.y, c.rT[u], lo);
+            lo = fma(l01.x, oml, lo);
+            double hi = fma(Tu, h45.x, h23.y);
+            hi = fma(Tu, hi, h23.x);
+            hi = fma(Tu, hi, h01.y);
+            hi = fma(Tu, hi, h6w.x);
+            hi = fma(h45.y, c.rT[u], hi);
+            hi = fma(h01.x, oml, hi);
+            const double g2 = Tu <= l6t.y ? lo : hi;
+            const double z = y[u] * h6w.y;
+            invW[u] += z;
+            *reinterpret_cast<double2 *>(sL + (size_t)k * 512 * PPL + 512 * u) = make_double2(z, exp2c(lc02[u] - g2));
+        }
+    }
+    if (warp == 0) {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u)
+            *reinterpret_cast<double2 *>(sL + (size_t)Ns * 512 * PPL + 512 * u) = make_double2(1.0, 1.0);
+    }
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) sred[(warp * PPL + u) * 32 + lane] = invW[u];
+    __syncthreads();
+    double rho[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
+        rho[u] = pi[u] / (CRF_R_GAS * c.T[u] * s);
+    }
+    for (int k = warp; k < Ns; k += W) {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) *reinterpret_cast<double *>(sL + (size_t)k * 512 * PPL + 512 * u) *= rho[u];  // C_k
+    }
+    stage_wait();
+    __syncthreads();
+
+    double om[MAXOWN][PPL];
+#pragma unroll
+    for (int s = 0; s < MAXOWN; ++s)
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) om[s][u] = 0.0;
+
+    const int nch = rs.n_chunks;
+    for (int ci = 0; ci < nch; ++ci) {
+        const int4 ch = __ldg(rs.chunk + ci);
+        const char *blk = sStage + (size_t)(ci & 1) * rs.stage_bytes;
+        if (ci + 1 < nch)
+            stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, rs.stage + __ldg(&rs.chunk[ci + 1].z),
+                        rs.stage_bytes, threadIdx.x, 32 * W);
+        const int count = ch.y;
+        const int o_slot = 48 * count, o_troe = (o_slot + 8 * Ns + 15) & ~15;
+        switch (ch.x) {
+        case 0: reaction_stage<W, PPL, 0, false>(blk, count, o_troe, sL, sQl, warp, c); break;
+        case 1: reaction_stage<W, PPL, 1, false>(blk, count, o_troe, sL, sQl, warp, c); break;
+        case 2: reaction_stage<W, PPL, 2, false>(blk, count, o_troe, sL, sQl, warp, c); break;
+        default: reaction_stage<W, PPL, 0, true>(blk, count, o_troe, sL, sQl, warp, c); break;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int s = 0; s < MAXOWN; ++s) {
+            const int k = warp + W * s;
+            if (k < Ns) {
+                const uint2 se = *reinterpret_cast<const uint2 *>(blk + o_slot + 8 * k);
+                for (unsigned e = se.x; e < se.y; e += 16) {
+                    const uint4 en = ldsu4(blk + e);
+                    const double nu = __hiloint2double((int)en.y, (int)en.x);
+#pragma unroll
+                    for (int u = 0; u < PPL; ++u)
+                        om[s][u] = fma(nu, *reinterpret_cast<const double *>(sQl + en.z + 256 * u), om[s][u]);
+                }
+            }
+        }
+        stage_wait();
+        __syncthreads();
+    }
+
+    // ---- store omega; a9: qdot = -sum_k h_k omega_k
+    double qd[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) qd[u] = 0.0;
+#pragma unroll
+    for (int s = 0; s < MAXOWN; ++s) {
+        const int k = warp + W * s;
+        if (k < Ns) {
+            const double2 *h = reinterpret_cast<const double2 *>(rs.hco + 16 * (size_t)k);
+            const double2 l01 = __ldg(h), l23 = __ldg(h + 1), l45 = __ldg(h + 2), l6t = __ldg(h + 3);
+            const double2 h01 = __ldg(h + 4), h23 = __ldg(h + 5), h45 = __ldg(h + 6);
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) {
+                const double Tu = c.T[u];
+                double lo = fma(Tu, l45.x, l23.y);
+                lo = fma(Tu, lo, l23.x);
+                lo = fma(Tu, lo, l01.y);
+                lo = fma(Tu, lo, l01.x);
+                lo = fma(l45.y, c.rT[u], lo);
+                double hi = fma(Tu, h45.x, h23.y);
+                hi = fma(Tu, hi, h23.x);
+                hi = fma(Tu, hi, h01.y);
+                hi = fma(Tu, hi, h01.x);
+                hi = fma(h45.y, c.rT[u], hi);
+                qd[u] = fma(-(Tu <= l6t.y ? lo : hi), om[s][u], qd[u]);
+            }
+            store_row<PPL>(omega + (int64_t)k * n, i0, n, vec, om[s]);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) sred[(warp * PPL + u) * 32 + lane] = qd[u];
+    __syncthreads();
+    if (warp == 0) {
+        double out[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) {
+            double s = 0.0;
+#pragma unroll
+            for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
+            out[u] = s * (CRF_R_GAS * c.T[u]);
+        }
+        store_row<PPL>(qdot, i0, n, vec, out);
+    }
+}
+
+template <int W, int PPL, int MAXOWN>
+cudaError_t launch_k(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
+                     double *qdot, cudaStream_t st)
+{
+    const size_t smem = (size_t)(m.Ns + 1) * 512 * PPL + (size_t)m.rs.Rc * 256 * PPL + 2 * (size_t)m.rs.stage_bytes;
+    cudaError_t e = cudaFuncSetAttribute(rates_smem_kernel<W, PPL, MAXOWN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem);
+    if (e != cudaSuccess) return e;
+    const int64_t per_block = 32 * PPL;
+    rates_smem_kernel<W, PPL, MAXOWN><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, p, Y, n,
+                                                                                                        omega, qdot);
+    crf_count_launch();
+    return cudaGetLastError();
+}
+
+template <int W, int PPL>
+cudaError_t launch_wp(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
+                      double *qdot, cudaStream_t st)
+{
+    const int own = (m.Ns + W - 1) / W;
+    if (own <= 4) return launch_k<W, PPL, 4>(m, T, p, Y, n, omega, qdot, st);
+    if (own <= 8) return launch_k<W, PPL, 8>(m, T, p, Y, n, omega, qdot, st);
+    if (own <= 16) return launch_k<W, PPL, 16>(m, T, p, Y, n, omega, qdot, st);
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
+                              double *omega, double *qdot, cudaStream_t st)
+{
+    const int key = m.rs.W * 10 + m.rs.PPL;
+    switch (key) {
+    case 41: return launch_wp<4, 1>(m, T, p, Y, n, omega, qdot, st);
+    case 42: return launch_wp<4, 2>(m, T, p, Y, n, omega, qdot, st);
+    case 81: return launch_wp<8, 1>(m, T, p, Y, n, omega, qdot, st);
+    case 82: return launch_wp<8, 2>(m, T, p, Y, n, omega, qdot, st);
+    case 161: return launch_wp<16, 1>(m, T, p, Y, n, omega, qdot, st);
+    case 162: return launch_wp<16, 2>(m, T, p, Y, n, omega, qdot, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
