@@ -196,7 +196,7 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
     rp.inc = reinterpret_cast<const double2 *>(base + rpo.inc);
     rp.troe = D(rpo.troe), rp.gco = D(rpo.gco), rp.hco = D(rpo.hco);
     RatesSmemPlan &rs = d.rs;
-    rs.W = rso.W, rs.PPL = rso.PPL, rs.Rc = rso.Rc, rs.n_chunks = rso.n_chunks, rs.stage_bytes = rso.stage_bytes;
+    rs.W = rso.W, rs.PPL = rso.PPL, rs.maxown = rso.maxown, rs.Rc = rso.Rc, rs.n_chunks = rso.n_chunks, rs.stage_bytes = rso.stage_bytes;
     rs.chunk = reinterpret_cast<const int4 *>(base + rso.chunk);
     rs.stage = base + rso.stage;
     rs.gco = D(rso.gco), rs.hco = D(rso.hco);

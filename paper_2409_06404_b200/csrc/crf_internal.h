@@ -46,13 +46,15 @@ struct RatesPlan {
 //                            u32 a0, a1, b0, b1 (byte offsets of the reactant/product rows in the state);
 //                            x0, x1 = third reactant/product rows (generic kinds) or offset/count of the
 //                            third-body list (kinds 1, 2)
-//   [48 count, +8 Ns)        per species (start, end) byte offsets of its incidence entries
-//   then (16-byte aligned)   Troe sets, 64 bytes per reaction (kind 2 only)
+//   [48 count, +(16 + 4 maxown) W)  per warp: u32 start of its incidence entries, 3 pad words, u32 end of the
+//                            entries of each owned species k = warp + W slot (entries are warp-major, slot-major)
+//   then                     Troe sets, 64 bytes per reaction (kind 2 only)
 //   then                     incidence entries {f64 nu, u32 byte offset of q_r, u32 0} and third-body
 //                            entries {f64 efficiency - 1, u32 state row offset, u32 0}
 struct RatesSmemPlan {
     int W;            // warps sharing a point group; 0 = no plan
     int PPL;          // points per lane (1 or 2)
+    int maxown;       // owned-species slots per warp the tables are laid out for (4, 8 or 16)
     int Rc;           // q buffer rows (max reactions per chunk)
     int n_chunks;
     int stage_bytes;  // largest chunk block, multiple of 16

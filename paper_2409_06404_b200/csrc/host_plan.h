@@ -32,7 +32,7 @@ struct RatesPlanOffsets {
 };
 
 struct RatesSmemPlanOffsets {
-    int W = 0, PPL = 0, Rc = 0, n_chunks = 0, stage_bytes = 0;
+    int W = 0, PPL = 0, maxown = 0, Rc = 0, n_chunks = 0, stage_bytes = 0;
     size_t chunk = 0, stage = 0, gco = 0, hco = 0;
 };
 

@@ -84,14 +84,15 @@ std::vector<Chunk> make_chunks(const Builder &B, int Rc)
     return out;
 }
 
-std::vector<unsigned char> chunk_block(const Builder &B, const Chunk &ch, int PPL)
+std::vector<unsigned char> chunk_block(const Builder &B, const Chunk &ch, int PPL, int W, int maxown)
 {
     const crf_tables *t = B.t;
     const int Ns = B.Ns, cnt = (int)ch.reactions.size();
     const unsigned row = 512u * PPL;   // bytes per species row of the (C, d) state
     const unsigned qrow = 256u * PPL;  // bytes per reaction row of the q buffer
     const size_t o_slot = 48 * (size_t)cnt;
-    const size_t o_troe = (o_slot + 8 * (size_t)Ns + 15) & ~size_t(15);
+    const size_t slot_row = 16 + 4 * (size_t)maxown;  // per warp: start, 3 pad words, end of each owned slot
+    const size_t o_troe = o_slot + slot_row * W;
     size_t o_list = o_troe + (ch.kind == 2 ? 64 * (size_t)cnt : 0);
     std::vector<unsigned char> v(o_list, 0);
     auto row_of = [&](int k) { return (unsigned)(k >= 0 ? k : Ns) * row; };  // row Ns: the dummy species (1, 1)
@@ -102,18 +103,21 @@ std::vector<unsigned char> chunk_block(const Builder &B, const Chunk &ch, int PP
         put(v, o + 8, y);
         return o;
     };
-    // incidence entries, species-major
-    for (int k = 0; k < Ns; ++k) {
-        const unsigned start = (unsigned)v.size();
-        for (int rl = 0; rl < cnt; ++rl) {
-            const int r = ch.reactions[rl];
-            int nu = 0;
-            for (int s = 0; s < 3; ++s) nu += (B.slot(t->prod, s, r) == k) - (B.slot(t->reac, s, r) == k);
-            if (nu != 0) append16((double)nu, (unsigned)rl * qrow);
+    // incidence entries: warp-major, then the warp's owned species k = w + W s in slot order
+    for (int w = 0; w < W; ++w) {
+        put(v, o_slot + slot_row * w, (unsigned)v.size());
+        for (int sl = 0; sl < maxown; ++sl) {
+            const int k = w + W * sl;
+            for (int rl = 0; rl < cnt && k < Ns; ++rl) {
+                const int r = ch.reactions[rl];
+                int nu = 0;
+                for (int s = 0; s < 3; ++s) nu += (B.slot(t->prod, s, r) == k) - (B.slot(t->reac, s, r) == k);
+                if (nu != 0) append16((double)nu, (unsigned)rl * qrow);
+            }
+            put(v, o_slot + slot_row * w + 16 + 4 * (size_t)sl, (unsigned)v.size());
         }
-        put(v, o_slot + 8 * (size_t)k, start);
-        put(v, o_slot + 8 * (size_t)k + 4, (unsigned)v.size());
     }
+    append16(0.0, 0u);  // the entry loop reads one entry ahead
     for (int rl = 0; rl < cnt; ++rl) {
         const int r = ch.reactions[rl];
         const size_t o = 48 * (size_t)rl;
@@ -167,15 +171,19 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
     // two chunk blocks.  CRF_RATES_W / CRF_RATES_PPL / CRF_RATES_RC override (tuning).
     auto budget = [](int W) { return (size_t)233472 / (16 / W) - 1024; };
     auto state = [&](int PPL) { return (size_t)(Ns + 1) * 512 * PPL; };
-    int PPL = env_int("CRF_RATES_PPL", Ns <= 32 ? 2 : 1);
+    // measured on C5 (Ns = 118): W/PPL = 16/2 11.2 ms, 8/1 13.8 ms, 16/1 14.4 ms -> large mechanisms take the
+    // whole SM as one block with two points per lane
+    const bool big = Ns > 64 && state(2) <= budget(16) * 6 / 10;
+    int PPL = env_int("CRF_RATES_PPL", Ns <= 32 || big ? 2 : 1);
     if (PPL != 1 && PPL != 2) PPL = 1;
-    int W = env_int("CRF_RATES_W", 0);
+    int W = env_int("CRF_RATES_W", big && PPL == 2 ? 16 : 0);
     if (W != 4 && W != 8 && W != 16) {
         W = 4;
         while (W < 16 && (state(PPL) > budget(W) * 6 / 10 || (Ns + W - 1) / W > 16)) W *= 2;
     }
     if ((Ns + W - 1) / W > 16 || state(PPL) + 2 * W * 256 * PPL > budget(W)) return o;
 
+    const int own = (Ns + W - 1) / W, maxown = own <= 4 ? 4 : (own <= 8 ? 8 : 16);
     const int step = 2 * W;
     int Rc = env_int("CRF_RATES_RC", 0);
     std::vector<Chunk> chunks;
@@ -187,14 +195,14 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
         blocks.clear();
         stage_bytes = 0;
         for (const Chunk &ch : chunks) {
-            blocks.push_back(chunk_block(B, ch, PPL));
+            blocks.push_back(chunk_block(B, ch, PPL, W, maxown));
             stage_bytes = std::max(stage_bytes, (blocks.back().size() + 15) & ~size_t(15));
         }
         Rc = cand;
         if (state(PPL) + (size_t)cand * 256 * PPL + 2 * stage_bytes <= budget(W)) break;
         if (cand == step) return o;  // does not fit at all
     }
-    o.W = W, o.PPL = PPL, o.Rc = Rc, o.n_chunks = (int)chunks.size(), o.stage_bytes = (int)stage_bytes;
+    o.W = W, o.PPL = PPL, o.maxown = maxown, o.Rc = Rc, o.n_chunks = (int)chunks.size(), o.stage_bytes = (int)stage_bytes;
 
     std::vector<int4> cdesc;
     std::vector<unsigned char> stage;

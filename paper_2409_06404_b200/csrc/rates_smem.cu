@@ -29,6 +29,13 @@
 
 namespace {
 
+// 2^f on [-1/2, 1/2], degree 9 (fastmath.cuh), in constant memory: the FP64 instructions take the
+// coefficients as constant-bank operands instead of occupying (and re-materialising) registers
+__constant__ double kExp2[10] = {0x1.000000000003dp+0, 0x1.62e42fefa39f7p-1,  0x1.ebfbdff8149f2p-3, 0x1.c6b08d7044119p-5,
+                                 0x1.3b2ab72b175eep-7, 0x1.5d87fe908f88ap-10, 0x1.43088e257f341p-13, 0x1.ffcb76789860fp-17,
+                                 0x1.63ef969a64d3cp-20, 0x1.b6571de2f2351p-24};
+__constant__ double kAtanh[9] = {1.0, 1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0, 1.0 / 17.0};
+
 __device__ __forceinline__ double exp2c(double y)
 {
     // crf::exp2_poly9 with the exponent clamped from below: an underflowing rate constant becomes a
@@ -37,16 +44,9 @@ __device__ __forceinline__ double exp2c(double y)
     const double t = __dadd_rn(y, magic);
     const int k = max(__double2loint(t), -1000);
     const double f = __dsub_rn(y, __dsub_rn(t, magic));
-    double p = 0x1.b6571de2f2351p-24;
-    p = fma(p, f, 0x1.63ef969a64d3cp-20);
-    p = fma(p, f, 0x1.ffcb76789860fp-17);
-    p = fma(p, f, 0x1.43088e257f341p-13);
-    p = fma(p, f, 0x1.5d87fe908f88ap-10);
-    p = fma(p, f, 0x1.3b2ab72b175eep-7);
-    p = fma(p, f, 0x1.c6b08d7044119p-5);
-    p = fma(p, f, 0x1.ebfbdff8149f2p-3);
-    p = fma(p, f, 0x1.62e42fefa39f7p-1);
-    p = fma(p, f, 0x1.000000000003dp+0);
+    double p = kExp2[9];
+#pragma unroll
+    for (int i = 8; i >= 0; --i) p = fma(p, f, kExp2[i]);
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
 }
 
@@ -68,16 +68,41 @@ __device__ __forceinline__ double log2_fast(double x)
     const double m = __hiloint2double(hi, __double2loint(x));
     const double s = (m - 1.0) * rcp_fast(m + 1.0);
     const double z = s * s;
-    double p = 1.0 / 17.0;
-    p = fma(p, z, 1.0 / 15.0);
-    p = fma(p, z, 1.0 / 13.0);
-    p = fma(p, z, 1.0 / 11.0);
-    p = fma(p, z, 1.0 / 9.0);
-    p = fma(p, z, 1.0 / 7.0);
-    p = fma(p, z, 1.0 / 5.0);
-    p = fma(p, z, 1.0 / 3.0);
-    p = fma(p, z, 1.0);
+    double p = kAtanh[8];
+#pragma unroll
+    for (int i = 7; i >= 0; --i) p = fma(p, z, kAtanh[i]);
     return fma(s * (2.0 * crf::kLog2e), p, (double)e);
+}
+
+// shared memory through 32-bit shared-window addresses (no generic-pointer arithmetic in the hot loops)
+__device__ __forceinline__ double2 lds_d2(unsigned a)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds_d(unsigned a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint4 lds_u4(unsigned a)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ unsigned lds_u(unsigned a)
+{
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts_d(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+__device__ __forceinline__ void sts_d2(unsigned a, double x, double y)
+{
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
 }
 
 template <int PPL>
@@ -302,7 +327,8 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
             stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, rs.stage + __ldg(&rs.chunk[ci + 1].z),
                         rs.stage_bytes, threadIdx.x, 32 * W);
         const int count = ch.y;
-        const int o_slot = 48 * count, o_troe = (o_slot + 8 * Ns + 15) & ~15;
+        constexpr int SLOT_ROW = 16 + 4 * MAXOWN;
+        const int o_slot = 48 * count, o_troe = o_slot + SLOT_ROW * W;
         switch (ch.x) {
         case 0: reaction_stage<W, PPL, 0, false>(blk, count, o_troe, sL, sQl, warp, c); break;
         case 1: reaction_stage<W, PPL, 1, false>(blk, count, o_troe, sL, sQl, warp, c); break;
@@ -310,17 +336,27 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         default: reaction_stage<W, PPL, 0, true>(blk, count, o_troe, sL, sQl, warp, c); break;
         }
         __syncthreads();
+        {
+            // the warp's entries are contiguous (slot-major); slot s ends at ends[s]; one entry is read ahead
+            const char *sr = blk + o_slot + SLOT_ROW * warp;
+            unsigned e = *reinterpret_cast<const unsigned *>(sr);
+            uint4 en = ldsu4(blk + e);
 #pragma unroll
-        for (int s = 0; s < MAXOWN; ++s) {
-            const int k = warp + W * s;
-            if (k < Ns) {
-                const uint2 se = *reinterpret_cast<const uint2 *>(blk + o_slot + 8 * k);
-                for (unsigned e = se.x; e < se.y; e += 16) {
-                    const uint4 en = ldsu4(blk + e);
-                    const double nu = __hiloint2double((int)en.y, (int)en.x);
+            for (int s4 = 0; s4 < MAXOWN; s4 += 4) {
+                const uint4 ends = ldsu4(sr + 16 + 4 * s4);
 #pragma unroll
-                    for (int u = 0; u < PPL; ++u)
-                        om[s][u] = fma(nu, *reinterpret_cast<const double *>(sQl + en.z + 256 * u), om[s][u]);
+                for (int j = 0; j < 4; ++j) {
+                    const int s = s4 + j;
+                    const unsigned end = j == 0 ? ends.x : (j == 1 ? ends.y : (j == 2 ? ends.z : ends.w));
+                    while (e < end) {
+                        const uint4 cur = en;
+                        e += 16;
+                        en = ldsu4(blk + e);
+                        const double nu = __hiloint2double((int)cur.y, (int)cur.x);
+#pragma unroll
+                        for (int u = 0; u < PPL; ++u)
+                            om[s][u] = fma(nu, *reinterpret_cast<const double *>(sQl + cur.z + 256 * u), om[s][u]);
+                    }
                 }
             }
         }
