@@ -6,16 +6,24 @@
 
 #define CRF_R_GAS 8314.46261815324  // J/(kmol K)
 
-// Plan of the tiled crf_mix_transport kernel (transport_tiled.cu): species padded to blocks of 8,
-// the pair triangle cut into 8x8 tiles, tiles dealt to the W warps that share 32 points in rounds
-// whose tiles touch disjoint species blocks (so the warps update disjoint rows of S).
+// Plan of the tiled crf_mix_transport kernel (transport_tiled.cu): species padded to blocks of 8, the pair
+// triangle cut into 8x8 tiles.  W warps share 32 PPL points; tiles are dealt to them in rounds whose tiles
+// touch disjoint species blocks (round-robin tournament over the blocks: a block's bye is its diagonal
+// tile), so the warps update disjoint rows of S.  A round's coefficients are one contiguous block that the
+// thread block copies global -> shared with cp.async while it works on the previous round.
 struct TransportPlan {
-    int W;         // warps per block (1, 2 or 4); 0 = no plan (generic kernel)
+    int W;         // warps per block (1, 2, 4 or 8); 0 = no plan (generic kernel)
+    int PPL;       // points per lane (1 or 2)
     int NsP, nb;   // padded species count (multiple of 8) and number of 8-blocks
-    int n_rounds;
+    int n_wilke;   // stage blocks of the Wilke phase (they come first in `rounds`)
+    int n_rounds;  // stage blocks (rounds) of the pair phase
+    int stage_bytes;          // largest stage block (multiple of 16)
+    const int4 *rounds;       // [n_wilke + n_rounds]: x = byte offset of the block in pair_coef, y = its bytes;
+                              //   Wilke blocks: z = first column block | pass << 8 | first panel << 16 |
+                              //   last panel << 17, w = column blocks nJ; layout [W][8 rows][8 nJ] of c_kj
     const int2 *sched;        // [n_rounds][W]: x = kind | jb << 8 | kb << 16 (kind 0 idle, 1 off-diagonal,
-                              //   2 diagonal), y = offset of the tile's coefficients in pair_coef (doubles)
-    const double *pair_coef;  // schedule order; per pair (c0,c1,c2,c3) of -log2(e) * ln D_jk fit; 0 for padding
+                              //   2 diagonal), y = byte offset of the tile's coefficients inside the round block
+    const unsigned char *pair_coef;  // per pair (c0,c1,c2,c3) of -log2(e) * ln D_jk fit; 0 for padding
     const double *wilke_cP;   // [NsP][NsP] c_kj = 1/sqrt(8 (1 + W_k/W_j)), 0 in padded rows/columns
     const double *sp;         // [NsP][12]: 0-3 ln(mu_k)/2 cubic, 4-7 ln(lambda_k) cubic, 8 W^-1/4, 9 W^1/2,
                               //   10 1/W (0 for padding), 11 unused

@@ -2,7 +2,7 @@
 // transport_tiled.cu (see the header comment there and TransportPlan in crf_internal.h).
 #include <cmath>
 #include <cstdint>
-#include <random>
+#include <cstdlib>
 
 #include "fastmath.cuh"
 #include "host_plan.h"
@@ -10,50 +10,46 @@
 namespace {
 
 struct Tile {
-    int jb, kb;
+    int kind, jb, kb;  // kind 1: off-diagonal tile (jb < kb), 2: diagonal tile (jb = kb)
 };
 
-// Rounds of at most W off-diagonal tiles whose species blocks are pairwise disjoint.  Greedy: each round
-// takes, among the tiles disjoint from those already chosen, the one whose blocks still have the most
-// tiles left (ties broken by a seeded shuffle); several seeds, fewest rounds wins.
-std::vector<std::vector<Tile>> schedule_offdiag(int nb, int W)
+int env_int(const char *name, int dflt)
 {
-    std::vector<std::vector<Tile>> best;
-    const int ntiles = nb * (nb - 1) / 2;
-    if (ntiles == 0) return best;
-    const size_t lower = (ntiles + W - 1) / W;
-    for (unsigned seed = 0; seed < 64; ++seed) {
-        std::mt19937 rng(seed);
-        std::vector<Tile> left;
-        for (int j = 0; j < nb; ++j)
-            for (int k = j + 1; k < nb; ++k) left.push_back({j, k});
-        std::shuffle(left.begin(), left.end(), rng);
-        std::vector<int> deg(nb, nb - 1);
-        std::vector<std::vector<Tile>> rounds;
-        while (!left.empty()) {
-            std::vector<Tile> rd;
-            std::vector<char> used(nb, 0);
-            while ((int)rd.size() < W) {
-                int pick = -1, score = -1;
-                for (size_t i = 0; i < left.size(); ++i) {
-                    const Tile &t = left[i];
-                    if (used[t.jb] || used[t.kb]) continue;
-                    const int s = deg[t.jb] + deg[t.kb];
-                    if (s > score) score = s, pick = (int)i;
-                }
-                if (pick < 0) break;
-                const Tile t = left[pick];
-                left.erase(left.begin() + pick);
-                used[t.jb] = used[t.kb] = 1;
-                --deg[t.jb], --deg[t.kb];
-                rd.push_back(t);
-            }
-            rounds.push_back(rd);
+    const char *s = std::getenv(name);
+    return s && *s ? std::atoi(s) : dflt;
+}
+
+// Rounds of at most W tiles whose species blocks are pairwise disjoint: the circle method of a round-robin
+// tournament over the nb blocks (an odd nb gets a dummy block; meeting the dummy is the block's bye, in
+// which it does its own diagonal tile).  nb odd: nb rounds of (nb-1)/2 off-diagonal tiles + 1 diagonal tile
+// cover the whole triangle; nb even: nb-1 rounds of nb/2 tiles, then the diagonal tiles.  Rounds with more
+// than W tiles are split.
+std::vector<std::vector<Tile>> schedule_rounds(int nb, int W)
+{
+    std::vector<std::vector<Tile>> rounds;
+    auto emit = [&](const std::vector<Tile> &tiles) {
+        for (size_t i = 0; i < tiles.size(); i += W)
+            rounds.emplace_back(tiles.begin() + i, tiles.begin() + std::min(tiles.size(), i + (size_t)W));
+    };
+    const int ne = nb + (nb & 1), m = ne - 1;  // m rotating blocks, block m is fixed (the dummy when nb is odd)
+    for (int r = 0; r < m && nb > 1; ++r) {
+        std::vector<Tile> tiles;
+        for (int i = 1; i < ne / 2; ++i) {
+            const int a = (r + i) % m, c = (r - i + m) % m;
+            tiles.push_back({1, std::min(a, c), std::max(a, c)});
         }
-        if (best.empty() || rounds.size() < best.size()) best = rounds;
-        if (best.size() == lower) break;
+        if (nb & 1)
+            tiles.push_back({2, r, r});
+        else
+            tiles.push_back({1, r, m});
+        emit(tiles);
     }
-    return best;
+    if (!(nb & 1) || nb == 1) {
+        std::vector<Tile> tiles;
+        for (int j = 0; j < nb; ++j) tiles.push_back({2, j, j});
+        emit(tiles);
+    }
+    return rounds;
 }
 
 }  // namespace
@@ -64,13 +60,18 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
     const int Ns = t->Ns;
     if (Ns < 17) return o;  // small mechanisms: generic kernel (a register-resident variant is the plan)
     const int nb = (Ns + 7) / 8, NsP = 8 * nb;
-    // warps per 32 points: enough warps per SM (>= 12 where the tile count allows), limited by
-    // 227 KB of shared memory per SM and by rounds needing W disjoint tiles (2W <= nb)
-    const size_t smem32 = sizeof(double) * 2 * (size_t)NsP * 32;
-    const int blocks_sm = (int)std::min<size_t>(12, (227 * 1024) / (smem32 + 1024 + 4 * 4 * 32 * 8));
-    int W = 1;
-    while (W < 4 && blocks_sm * W < 12 && 2 * (2 * W) <= nb) W *= 2;
-    o.W = W, o.NsP = NsP, o.nb = nb;
+    // warps per point group: one per tile of a round-robin round (nb odd: (nb+1)/2, nb even: nb/2), at most 8;
+    // points per lane: 1 (16 warps per SM at 128 registers) or 2 (8 warps per SM, every coefficient load
+    // serves two points).  CRF_TRANSPORT_W / CRF_TRANSPORT_PPL override (tuning).
+    const int per_round = std::max(1, (nb + (nb & 1)) / 2);
+    int W = env_int("CRF_TRANSPORT_W", 0);
+    if (W != 1 && W != 2 && W != 4 && W != 8) {
+        W = 1;
+        while (W < 8 && W < per_round) W *= 2;
+    }
+    int PPL = env_int("CRF_TRANSPORT_PPL", 1);
+    if (PPL != 1 && PPL != 2) PPL = 1;
+    o.W = W, o.PPL = PPL, o.NsP = NsP, o.nb = nb;
 
     const int npair = Ns * (Ns + 1) / 2;
     auto pair_index = [&](int j, int k) {
@@ -82,31 +83,45 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
             dst.push_back(j < Ns && k < Ns ? -crf::kLog2e * t->D_c[(size_t)c * npair + pair_index(j, k)] : 0.0);
     };
     std::vector<int2> sched;
+    std::vector<int4> rdesc;
     std::vector<double> coef;
-    auto rounds = schedule_offdiag(nb, W);
-    for (auto &rd : rounds)
+    size_t stage_bytes = 16;
+    // Wilke stage blocks: pass p covers the row blocks p W .. p W + W - 1 (one per warp), a panel covers up to
+    // kPanel column blocks; block layout [W][8 rows][8 nJ columns] of c_kj (0 in padded rows/columns)
+    const int kPanel = 3, npass = (nb + W - 1) / W;
+    for (int ps = 0; ps < npass; ++ps)
+        for (int J0 = 0; J0 < nb; J0 += kPanel) {
+            const int nJ = std::min(kPanel, nb - J0);
+            const size_t start = coef.size();
+            for (int w = 0; w < W; ++w)
+                for (int a = 0; a < 8; ++a)
+                    for (int c = 0; c < 8 * nJ; ++c) {
+                        const int k = 8 * (ps * W + w) + a, j = 8 * J0 + c;
+                        coef.push_back(k < Ns && j < Ns ? 1.0 / std::sqrt(8.0 * (1.0 + t->W[k] / t->W[j])) : 0.0);
+                    }
+            const int flags = J0 | ps << 8 | (J0 == 0) << 16 | (J0 + nJ == nb) << 17;
+            rdesc.push_back(make_int4((int)(8 * start), (int)(8 * (coef.size() - start)), flags, nJ));
+            stage_bytes = std::max(stage_bytes, 8 * (coef.size() - start));
+        }
+    o.n_wilke = (int)rdesc.size();
+    for (auto &rd : schedule_rounds(nb, W)) {
+        const size_t start = coef.size();
         for (int w = 0; w < W; ++w) {
             if (w >= (int)rd.size()) {
                 sched.push_back(make_int2(0, 0));
                 continue;
             }
             const Tile &tl = rd[w];
-            sched.push_back(make_int2(1 | tl.jb << 8 | tl.kb << 16, (int)coef.size()));
+            sched.push_back(make_int2(tl.kind | tl.jb << 8 | tl.kb << 16, (int)(8 * (coef.size() - start))));
             for (int a = 0; a < 8; ++a)
-                for (int c = 0; c < 8; ++c) put_pair(coef, 8 * tl.jb + a, 8 * tl.kb + c);
+                for (int c = tl.kind == 1 ? 0 : a + 1; c < 8; ++c) put_pair(coef, 8 * tl.jb + a, 8 * tl.kb + c);
         }
-    for (int j0 = 0; j0 < nb; j0 += W)
-        for (int w = 0; w < W; ++w) {
-            const int jb = j0 + w;
-            if (jb >= nb) {
-                sched.push_back(make_int2(0, 0));
-                continue;
-            }
-            sched.push_back(make_int2(2 | jb << 8 | jb << 16, (int)coef.size()));
-            for (int a = 0; a < 8; ++a)
-                for (int c = a + 1; c < 8; ++c) put_pair(coef, 8 * jb + a, 8 * jb + c);
-        }
-    o.n_rounds = (int)(sched.size() / W);
+        if (coef.size() & 1) coef.push_back(0.0);
+        rdesc.push_back(make_int4((int)(8 * start), (int)(8 * (coef.size() - start)), 0, 0));
+        stage_bytes = std::max(stage_bytes, 8 * (coef.size() - start));
+    }
+    o.n_rounds = (int)rdesc.size() - o.n_wilke;
+    o.stage_bytes = (int)stage_bytes;
 
     std::vector<double> cP((size_t)NsP * NsP, 0.0), sp((size_t)NsP * 12, 0.0), dd((size_t)Ns * 4);
     for (int k = 0; k < Ns; ++k) {
@@ -121,6 +136,6 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
         s[9] = std::sqrt(t->W[k]);
         s[10] = 1.0 / t->W[k];
     }
-    o.sched = b.add(sched), o.pair_coef = b.add(coef), o.wilke_cP = b.add(cP), o.sp = b.add(sp), o.Ddiag = b.add(dd);
+    o.rounds = b.add(rdesc), o.sched = b.add(sched), o.pair_coef = b.add(coef), o.wilke_cP = b.add(cP), o.sp = b.add(sp), o.Ddiag = b.add(dd);
     return o;
 }

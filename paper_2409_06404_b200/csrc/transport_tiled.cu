@@ -10,7 +10,10 @@
 // points: the pair triangle is cut into 8x8 species tiles, a tile is evaluated entirely in registers
 // (Z_j[8], Z_k[8], S_j[8], S_k[8] -> 64 independent exp chains of ILP), and tiles are dealt to the
 // warps in rounds whose tiles touch disjoint species blocks, so the shared S rows are updated without
-// atomics; one __syncthreads per round.  Each unordered pair is evaluated once:
+// atomics; one __syncthreads per round (round-robin tournament over the blocks, plan_transport.cu).  A round's
+// coefficients are copied global -> shared with cp.async while the previous round is evaluated, so the pair
+// loop reads every coefficient as a warp-uniform shared-memory load.  A lane may carry PPL = 2 adjacent
+// points: each coefficient load then serves two points.  Each unordered pair is evaluated once:
 // e = 1/D_jk(p_ref) = 2^(cubic(ln T)) with -log2(e) folded into the table, S_j += Z_k e, S_k += Z_j e.
 //
 // Wilke: Phi_kj = c_kj (1 + a_k/a_j)^2, a_k = sqrt(mu_k) W_k^(-1/4), expanded so that the O(Ns^2) part is
@@ -33,195 +36,327 @@ __device__ __forceinline__ double cubic4(const double *__restrict__ c, double x)
     return fma(x, fma(x, fma(x, hi.y, hi.x), lo.y), lo.x);
 }
 
-// off-diagonal tile: species blocks jb < kb, 64 pairs
-__device__ __forceinline__ void tile_offdiag(const double *__restrict__ cf, double L, const double *sZ, double *sS,
-                                             int jb, int kb, int lane)
+// state rows: [species][PPL][32] doubles; sZl / sSl point at this lane's column
+#define ROW(k, u) (((k) * PPL + (u)) * 32)
+
+// off-diagonal tile: species blocks jb < kb, 64 pairs; cf: the tile's coefficients in shared memory
+template <int PPL>
+__device__ __forceinline__ void tile_offdiag(const double2 *cf, const double (&L)[PPL], const double *sZl, double *sSl,
+                                             int jb, int kb)
 {
-    double zj[8], zk[8], sj[8], sk[8];
+    double zj[PPL][8], zk[PPL][8], sj[PPL][8], sk[PPL][8];
 #pragma unroll
-    for (int a = 0; a < 8; ++a) {
-        zj[a] = sZ[(8 * jb + a) * 32 + lane];
-        zk[a] = sZ[(8 * kb + a) * 32 + lane];
-        sj[a] = 0.0;
-        sk[a] = 0.0;
-    }
+    for (int u = 0; u < PPL; ++u)
+#pragma unroll
+        for (int a = 0; a < 8; ++a) {
+            zj[u][a] = sZl[ROW(8 * jb + a, u)];
+            zk[u][a] = sZl[ROW(8 * kb + a, u)];
+            sj[u][a] = 0.0;
+            sk[u][a] = 0.0;
+        }
 #pragma unroll
     for (int a = 0; a < 8; ++a) {
 #pragma unroll
         for (int b = 0; b < 8; ++b) {
-            const double e = exp2_poly9(cubic4(cf + 4 * (8 * a + b), L));
-            sj[a] = fma(zk[b], e, sj[a]);
-            sk[b] = fma(zj[a], e, sk[b]);
+            const double2 lo = cf[2 * (8 * a + b)], hi = cf[2 * (8 * a + b) + 1];
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) {
+                const double e = exp2_poly9(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x));
+                sj[u][a] = fma(zk[u][b], e, sj[u][a]);
+                sk[u][b] = fma(zj[u][a], e, sk[u][b]);
+            }
         }
     }
 #pragma unroll
-    for (int a = 0; a < 8; ++a) {
-        sS[(8 * jb + a) * 32 + lane] += sj[a];
-        sS[(8 * kb + a) * 32 + lane] += sk[a];
-    }
+    for (int u = 0; u < PPL; ++u)
+#pragma unroll
+        for (int a = 0; a < 8; ++a) {
+            sSl[ROW(8 * jb + a, u)] += sj[u][a];
+            sSl[ROW(8 * kb + a, u)] += sk[u][a];
+        }
 }
 
 // diagonal tile: pairs a < b inside block jb, 28 pairs
-__device__ __forceinline__ void tile_diag(const double *__restrict__ cf, double L, const double *sZ, double *sS, int jb,
-                                          int lane)
+template <int PPL>
+__device__ __forceinline__ void tile_diag(const double2 *cf, const double (&L)[PPL], const double *sZl, double *sSl, int jb)
 {
-    double z[8], s[8];
+    double z[PPL][8], s[PPL][8];
 #pragma unroll
-    for (int a = 0; a < 8; ++a) {
-        z[a] = sZ[(8 * jb + a) * 32 + lane];
-        s[a] = 0.0;
-    }
+    for (int u = 0; u < PPL; ++u)
+#pragma unroll
+        for (int a = 0; a < 8; ++a) {
+            z[u][a] = sZl[ROW(8 * jb + a, u)];
+            s[u][a] = 0.0;
+        }
     int q = 0;
 #pragma unroll
     for (int a = 0; a < 8; ++a) {
 #pragma unroll
         for (int b = a + 1; b < 8; ++b, ++q) {
-            const double e = exp2_poly9(cubic4(cf + 4 * q, L));
-            s[a] = fma(z[b], e, s[a]);
-            s[b] = fma(z[a], e, s[b]);
+            const double2 lo = cf[2 * q], hi = cf[2 * q + 1];
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) {
+                const double e = exp2_poly9(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x));
+                s[u][a] = fma(z[u][b], e, s[u][a]);
+                s[u][b] = fma(z[u][a], e, s[u][b]);
+            }
         }
     }
 #pragma unroll
-    for (int a = 0; a < 8; ++a) sS[(8 * jb + a) * 32 + lane] += s[a];
+    for (int u = 0; u < PPL; ++u)
+#pragma unroll
+        for (int a = 0; a < 8; ++a) sSl[ROW(8 * jb + a, u)] += s[u][a];
 }
 
-template <int W>
-__global__ void __launch_bounds__(32 * W, 12 / W)
+__device__ __forceinline__ void stage_async(unsigned char *dst, const unsigned char *src, int bytes, int tid, int nthreads)
+{
+    for (int o = tid * 16; o < bytes; o += nthreads * 16) {
+        const unsigned d = (unsigned)__cvta_generic_to_shared(dst + o);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src + o) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void stage_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// the PPL points of a lane are adjacent: i0, i0 + 1 (one 128-bit access per row when n is even)
+template <int PPL>
+__device__ __forceinline__ void load_row(const double *__restrict__ row, int64_t i0, int64_t n, bool vec, double (&v)[PPL])
+{
+    if (PPL == 2 && vec && i0 + 1 < n) {
+        const double2 t = *reinterpret_cast<const double2 *>(row + i0);
+        v[0] = t.x, v[PPL - 1] = t.y;
+    } else {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) v[u] = row[min(i0 + u, n - 1)];
+    }
+}
+template <int PPL>
+__device__ __forceinline__ void store_row(double *__restrict__ row, int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
+{
+    if (PPL == 2 && vec && i0 + 1 < n) {
+        *reinterpret_cast<double2 *>(row + i0) = make_double2(v[0], v[PPL - 1]);
+    } else {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u)
+            if (i0 + u < n) row[i0 + u] = v[u];
+    }
+}
+
+template <int W, int PPL>
+__global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
     transport_tiled_kernel(DevTables m, const double *__restrict__ T, const double *__restrict__ Y, int64_t n,
                            double *__restrict__ mu, double *__restrict__ lambda, double *__restrict__ rhoD)
 {
-    extern __shared__ double sm[];
+    extern __shared__ double2 sm2[];
+    double *sm = reinterpret_cast<double *>(sm2);
     const TransportPlan &tp = m.tp;
     const int Ns = m.Ns, NsP = tp.NsP, nb = tp.nb;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double *sZ = sm;                     // [NsP][32]  Z_k = Y_k / W_k
-    double *sS = sm + (size_t)NsP * 32;  // [NsP][32]  1/a_k during the Wilke phase, then the diffusion sums
-    double *sred = sS + (size_t)NsP * 32;  // [4][W][32] partial sums of the warps
+    double *sZ = sm;                             // [NsP][PPL][32]  Z_k = Y_k / W_k
+    double *sS = sZ + (size_t)NsP * PPL * 32;    // [NsP][PPL][32]  1/a_k during the Wilke phase, then the diffusion sums
+    double *sred = sS + (size_t)NsP * PPL * 32;  // [4][W][PPL][32] partial sums of the warps
+    unsigned char *sStage = reinterpret_cast<unsigned char *>(sred + 4 * W * PPL * 32);  // [2][stage_bytes]
+    const double *sZl = sZ + lane;
+    double *sSl = sS + lane;
 
-    const int64_t i = (int64_t)blockIdx.x * 32 + lane;
-    const bool valid = i < n;
-    const int64_t ic = valid ? i : n - 1;  // lanes past the end recompute the last point and store nothing
-    const double Ti = T[ic];
-    const double L = log(Ti);
+    {
+        const int4 r0 = __ldg(tp.rounds);
+        stage_async(sStage, tp.pair_coef + r0.x, r0.y, threadIdx.x, 32 * W);
+    }
+
+    const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * PPL;
+    const bool vec = (n & 1) == 0;
+    double Ti[PPL], L[PPL];
+    load_row<PPL>(T, i0, n, vec, Ti);
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) L[u] = log(Ti[u]);
 
     // ---- a1, a10, a12: Z_k, species fits, conductivity sums; warp w takes species w, w+W, ...
-    double invW = 0.0, sum_a = 0.0, sum_h = 0.0;
+    double invW[PPL], sum_a[PPL], sum_h[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) invW[u] = sum_a[u] = sum_h[u] = 0.0;
     for (int k = warp; k < NsP; k += W) {
-        double z = 0.0, r = 0.0;
+        double z[PPL], r[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) z[u] = r[u] = 0.0;
         if (k < Ns) {
             const double *sp = tp.sp + 12 * k;
-            z = Y[(int64_t)k * n + ic] * __ldg(sp + 10);
-            const double smu = exp(cubic4(sp, L));       // sqrt(mu_k)
-            const double lam = exp(cubic4(sp + 4, L));   // lambda_k
-            r = 1.0 / (smu * __ldg(sp + 8));             // 1/a_k
-            invW += z;
-            sum_a = fma(z, lam, sum_a);
-            sum_h += z / lam;
-        }
-        sZ[k * 32 + lane] = z;
-        sS[k * 32 + lane] = r;
-    }
-    sred[(0 * W + warp) * 32 + lane] = invW;
-    sred[(1 * W + warp) * 32 + lane] = sum_a;
-    sred[(2 * W + warp) * 32 + lane] = sum_h;
-    __syncthreads();
-
-    // ---- a11: Wilke, row blocks dealt to the warps
-    double mu_p = 0.0;
-    for (int I = warp; I < nb; I += W) {
-        double A[8], B[8], C[8];
+            double y[PPL];
+            load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y);
 #pragma unroll
-        for (int a = 0; a < 8; ++a) A[a] = B[a] = C[a] = 0.0;
-        for (int J = 0; J < nb; ++J) {
-            double u0[8], u1[8], u2[8];
-#pragma unroll
-            for (int b = 0; b < 8; ++b) {
-                u0[b] = sZ[(8 * J + b) * 32 + lane];
-                const double r = sS[(8 * J + b) * 32 + lane];
-                u1[b] = u0[b] * r;
-                u2[b] = u1[b] * r;
+            for (int u = 0; u < PPL; ++u) {
+                z[u] = y[u] * __ldg(sp + 10);
+                const double smu = exp(cubic4(sp, L[u]));      // sqrt(mu_k)
+                const double lam = exp(cubic4(sp + 4, L[u]));  // lambda_k
+                r[u] = 1.0 / (smu * __ldg(sp + 8));            // 1/a_k
+                invW[u] += z[u];
+                sum_a[u] = fma(z[u], lam, sum_a[u]);
+                sum_h[u] += z[u] / lam;
             }
-            const double *c = tp.wilke_cP + (size_t)(8 * I) * NsP + 8 * J;
+        }
 #pragma unroll
-            for (int a = 0; a < 8; ++a) {
+        for (int u = 0; u < PPL; ++u) {
+            sZ[ROW(k, u) + lane] = z[u];
+            sS[ROW(k, u) + lane] = r[u];
+        }
+    }
 #pragma unroll
-                for (int b = 0; b < 8; b += 2) {
-                    const double2 cc = __ldg(reinterpret_cast<const double2 *>(c + (size_t)a * NsP + b));
-                    A[a] = fma(cc.x, u0[b], A[a]);
-                    B[a] = fma(cc.x, u1[b], B[a]);
-                    C[a] = fma(cc.x, u2[b], C[a]);
-                    A[a] = fma(cc.y, u0[b + 1], A[a]);
-                    B[a] = fma(cc.y, u1[b + 1], B[a]);
-                    C[a] = fma(cc.y, u2[b + 1], C[a]);
+    for (int u = 0; u < PPL; ++u) {
+        sred[((0 * W + warp) * PPL + u) * 32 + lane] = invW[u];
+        sred[((1 * W + warp) * PPL + u) * 32 + lane] = sum_a[u];
+        sred[((2 * W + warp) * PPL + u) * 32 + lane] = sum_h[u];
+    }
+
+    // ---- a11: Wilke.  Pass ps gives warp w the row block I = ps W + w; the c_kj of a pass arrive in panels of
+    // column blocks (stage blocks, plan_transport.cu); the block after the last panel is pair round 0.
+    double mu_p[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) mu_p[u] = 0.0;
+    const int nwk = tp.n_wilke;
+    {
+        double A[PPL][8], B[PPL][8], C[PPL][8];
+        for (int s = 0; s < nwk; ++s) {
+            stage_wait();
+            __syncthreads();  // block s has landed; everyone is done with block s - 1
+            const int4 ds = __ldg(tp.rounds + s), d1 = __ldg(tp.rounds + s + 1);
+            stage_async(sStage + (size_t)((s + 1) & 1) * tp.stage_bytes, tp.pair_coef + d1.x, d1.y, threadIdx.x, 32 * W);
+            const int J0 = ds.z & 0xff, I = ((ds.z >> 8) & 0xff) * W + warp, nJ = ds.w;
+            if (I >= nb) continue;
+            if (ds.z & (1 << 16)) {
+#pragma unroll
+                for (int u = 0; u < PPL; ++u)
+#pragma unroll
+                    for (int a = 0; a < 8; ++a) A[u][a] = B[u][a] = C[u][a] = 0.0;
+            }
+            const int ld = 8 * nJ;  // row length of the slab
+            const double *cw = reinterpret_cast<const double *>(sStage + (size_t)(s & 1) * tp.stage_bytes) + warp * 8 * ld;
+            for (int jj = 0; jj < nJ; ++jj) {
+#pragma unroll
+                for (int u = 0; u < PPL; ++u) {
+                    double u0[8], u1[8], u2[8];
+#pragma unroll
+                    for (int b = 0; b < 8; ++b) {
+                        u0[b] = sZl[ROW(8 * (J0 + jj) + b, u)];
+                        const double r = sSl[ROW(8 * (J0 + jj) + b, u)];
+                        u1[b] = u0[b] * r;
+                        u2[b] = u1[b] * r;
+                    }
+#pragma unroll
+                    for (int a = 0; a < 8; ++a) {
+#pragma unroll
+                        for (int b = 0; b < 8; b += 2) {
+                            const double2 cc = *reinterpret_cast<const double2 *>(cw + a * ld + 8 * jj + b);
+                            A[u][a] = fma(cc.x, u0[b], A[u][a]);
+                            B[u][a] = fma(cc.x, u1[b], B[u][a]);
+                            C[u][a] = fma(cc.x, u2[b], C[u][a]);
+                            A[u][a] = fma(cc.y, u0[b + 1], A[u][a]);
+                            B[u][a] = fma(cc.y, u1[b + 1], B[u][a]);
+                            C[u][a] = fma(cc.y, u2[b + 1], C[u][a]);
+                        }
+                    }
+                }
+            }
+            if (ds.z & (1 << 17)) {
+#pragma unroll
+                for (int a = 0; a < 8; ++a) {
+                    const int k = 8 * I + a;
+                    if (k < Ns) {
+                        const double wk = __ldg(tp.sp + 12 * k + 9);
+#pragma unroll
+                        for (int u = 0; u < PPL; ++u) {
+                            const double ak = 1.0 / sSl[ROW(k, u)];
+                            const double ak2 = ak * ak;
+                            const double den = fma(ak2, C[u][a], fma(ak + ak, B[u][a], A[u][a]));
+                            mu_p[u] += sZl[ROW(k, u)] * (ak2 * wk) / den;
+                        }
+                    }
                 }
             }
         }
-#pragma unroll
-        for (int a = 0; a < 8; ++a) {
-            const int k = 8 * I + a;
-            if (k < Ns) {
-                const double ak = 1.0 / sS[k * 32 + lane];
-                const double ak2 = ak * ak;
-                const double den = fma(ak2, C[a], fma(ak + ak, B[a], A[a]));
-                mu_p += sZ[k * 32 + lane] * (ak2 * __ldg(tp.sp + 12 * k + 9)) / den;
-            }
-        }
     }
-    sred[(3 * W + warp) * 32 + lane] = mu_p;
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) sred[((3 * W + warp) * PPL + u) * 32 + lane] = mu_p[u];
     __syncthreads();  // every warp is done reading 1/a_k
-    for (int k = warp; k < NsP; k += W) sS[k * 32 + lane] = 0.0;
-    if (warp == 0 && valid) {
-        double iw = 0.0, sa = 0.0, sh = 0.0, mm = 0.0;
+    for (int k = warp; k < NsP; k += W)
 #pragma unroll
-        for (int w = 0; w < W; ++w) {
-            iw += sred[(0 * W + w) * 32 + lane];
-            sa += sred[(1 * W + w) * 32 + lane];
-            sh += sred[(2 * W + w) * 32 + lane];
-            mm += sred[(3 * W + w) * 32 + lane];
-        }
-        // lambda = (sum X lambda_k + 1/sum X/lambda_k)/2 with X = Z Wbar = Z / iw ; mu: Wbar cancels
-        lambda[i] = 0.5 * (sa / iw + iw / sh);
-        mu[i] = mm;
+        for (int u = 0; u < PPL; ++u) sS[ROW(k, u) + lane] = 0.0;
+    double iw[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) {
+        iw[u] = 0.0;
+#pragma unroll
+        for (int w = 0; w < W; ++w) iw[u] += sred[((0 * W + w) * PPL + u) * 32 + lane];
     }
+    if (warp == 0) {
+        double lam_o[PPL], mu_o[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) {
+            double sa = 0.0, sh = 0.0, mm = 0.0;
+#pragma unroll
+            for (int w = 0; w < W; ++w) {
+                sa += sred[((1 * W + w) * PPL + u) * 32 + lane];
+                sh += sred[((2 * W + w) * PPL + u) * 32 + lane];
+                mm += sred[((3 * W + w) * PPL + u) * 32 + lane];
+            }
+            // lambda = (sum X lambda_k + 1/sum X/lambda_k)/2 with X = Z Wbar = Z / iw ; mu: Wbar cancels
+            lam_o[u] = 0.5 * (sa / iw[u] + iw[u] / sh);
+            mu_o[u] = mm;
+        }
+        store_row<PPL>(lambda, i0, n, vec, lam_o);
+        store_row<PPL>(mu, i0, n, vec, mu_o);
+    }
+    stage_wait();
     __syncthreads();
 
-    // ---- a13: binary pairs, tiles in rounds
-    for (int rd = 0; rd < tp.n_rounds; ++rd) {
+    // ---- a13: binary pairs, tiles in rounds; round rd+1 is staged while round rd is evaluated
+    const int nrd = tp.n_rounds;
+    for (int rd = 0; rd < nrd; ++rd) {
+        const unsigned char *blk = sStage + (size_t)((nwk + rd) & 1) * tp.stage_bytes;
+        if (rd + 1 < nrd) {
+            const int4 r1 = __ldg(tp.rounds + nwk + rd + 1);
+            stage_async(sStage + (size_t)((nwk + rd + 1) & 1) * tp.stage_bytes, tp.pair_coef + r1.x, r1.y, threadIdx.x, 32 * W);
+        }
         const int2 d = __ldg(tp.sched + rd * W + warp);
         const int kind = d.x & 0xff, jb = (d.x >> 8) & 0xff, kb = (d.x >> 16) & 0xff;
-        const double *cf = tp.pair_coef + d.y;
+        const double2 *cf = reinterpret_cast<const double2 *>(blk + d.y);
         if (kind == 1)
-            tile_offdiag(cf, L, sZ, sS, jb, kb, lane);
+            tile_offdiag<PPL>(cf, L, sZl, sSl, jb, kb);
         else if (kind == 2)
-            tile_diag(cf, L, sZ, sS, jb, lane);
-        if (W > 1) __syncthreads();
+            tile_diag<PPL>(cf, L, sZl, sSl, jb);
+        stage_wait();
+        __syncthreads();
     }
 
     // ---- rho D_km = p_ref (1 - Y_k) / (R T S_k); pure species: rho D_kk = Wbar p_ref D_kk(p_ref) / (R T)
-    const double f = m.p_ref / (CRF_R_GAS * Ti);
-    double iw = 0.0;
+    double f[PPL];
 #pragma unroll
-    for (int w = 0; w < W; ++w) iw += sred[(0 * W + w) * 32 + lane];
+    for (int u = 0; u < PPL; ++u) f[u] = m.p_ref / (CRF_R_GAS * Ti[u]);
     for (int k = warp; k < Ns; k += W) {
-        const double s = sS[k * 32 + lane];
-        double v;
-        if (s == 0.0)
-            v = f / iw * exp(cubic4(tp.Ddiag + 4 * k, L));
-        else
-            v = f * (1.0 - Y[(int64_t)k * n + ic]) / s;
-        if (valid) rhoD[(int64_t)k * n + i] = v;
+        double y[PPL], v[PPL];
+        load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y);
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) {
+            const double s = sS[ROW(k, u) + lane];
+            if (s == 0.0)
+                v[u] = f[u] / iw[u] * exp(cubic4(tp.Ddiag + 4 * k, L[u]));
+            else
+                v[u] = f[u] * (1.0 - y[u]) / s;
+        }
+        store_row<PPL>(rhoD + (int64_t)k * n, i0, n, vec, v);
     }
 }
 
-template <int W>
+template <int W, int PPL>
 cudaError_t launch_w(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu, double *lambda,
                      double *rhoD, cudaStream_t st)
 {
-    const size_t smem = sizeof(double) * ((size_t)2 * m.tp.NsP * 32 + 4 * W * 32);
-    cudaError_t e = cudaFuncSetAttribute(transport_tiled_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    const size_t smem = sizeof(double) * ((size_t)2 * m.tp.NsP + 4 * W) * PPL * 32 + 2 * (size_t)m.tp.stage_bytes;
+    cudaError_t e = cudaFuncSetAttribute(transport_tiled_kernel<W, PPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem);
     if (e != cudaSuccess) return e;
-    transport_tiled_kernel<W><<<(unsigned)((n + 31) / 32), 32 * W, smem, st>>>(m, T, Y, n, mu, lambda, rhoD);
+    const int64_t per_block = 32 * PPL;
+    transport_tiled_kernel<W, PPL><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, Y, n, mu,
+                                                                                                     lambda, rhoD);
     crf_count_launch();
     return cudaGetLastError();
 }
@@ -231,10 +366,15 @@ cudaError_t launch_w(const DevTables &m, const double *T, const double *Y, int64
 cudaError_t launch_transport_tiled(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu,
                                    double *lambda, double *rhoD, cudaStream_t st)
 {
-    switch (m.tp.W) {
-    case 1: return launch_w<1>(m, T, Y, n, mu, lambda, rhoD, st);
-    case 2: return launch_w<2>(m, T, Y, n, mu, lambda, rhoD, st);
-    case 4: return launch_w<4>(m, T, Y, n, mu, lambda, rhoD, st);
+    switch (m.tp.W * 10 + m.tp.PPL) {
+    case 11: return launch_w<1, 1>(m, T, Y, n, mu, lambda, rhoD, st);
+    case 21: return launch_w<2, 1>(m, T, Y, n, mu, lambda, rhoD, st);
+    case 41: return launch_w<4, 1>(m, T, Y, n, mu, lambda, rhoD, st);
+    case 81: return launch_w<8, 1>(m, T, Y, n, mu, lambda, rhoD, st);
+    case 12: return launch_w<1, 2>(m, T, Y, n, mu, lambda, rhoD, st);
+    case 22: return launch_w<2, 2>(m, T, Y, n, mu, lambda, rhoD, st);
+    case 42: return launch_w<4, 2>(m, T, Y, n, mu, lambda, rhoD, st);
+    case 82: return launch_w<8, 2>(m, T, Y, n, mu, lambda, rhoD, st);
     default: return cudaErrorInvalidValue;
     }
 }
