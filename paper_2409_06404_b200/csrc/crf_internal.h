@@ -25,7 +25,7 @@ struct TransportPlan {
                               //   2 diagonal), y = byte offset of the tile's coefficients inside the round block
     const unsigned char *pair_coef;  // per pair (c0,c1,c2,c3) of -log2(e) * ln D_jk fit; 0 for padding
     const double *wilke_cP;   // [NsP][NsP] c_kj = 1/sqrt(8 (1 + W_k/W_j)), 0 in padded rows/columns
-    const double *sp;         // [NsP][12]: 0-3 ln(mu_k)/2 cubic, 4-7 ln(lambda_k) cubic, 8 W^-1/4, 9 W^1/2,
+    const double *sp;         // [NsP][12]: 0-3 -log2(e) ln(mu_k)/2 cubic, 4-7 log2(e) ln(lambda_k) cubic, 8 W^1/4, 9 W^1/2,
                               //   10 1/W (0 for padding), 11 unused
     const double *Ddiag;      // [Ns][4] ln D_kk cubic (pure-species guard)
 };

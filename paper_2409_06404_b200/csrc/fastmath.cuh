@@ -36,6 +36,15 @@ __device__ __forceinline__ double exp2_poly9(double y)
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
 }
 
+// 1/x for normal x: MUFU.RCP64H seed (relative error < 2^-20) and one cubic Newton step (error ~ 2^-60 + rounding)
+__device__ __forceinline__ double rcp_newton(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    return fma(y, fma(e, e, e), y);
+}
+
 constexpr double kLog2e = 1.4426950408889634074;
 
 }  // namespace crf

@@ -128,11 +128,11 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
         for (int j = 0; j < Ns; ++j) cP[(size_t)k * NsP + j] = 1.0 / std::sqrt(8.0 * (1.0 + t->W[k] / t->W[j]));
         double *s = sp.data() + 12 * (size_t)k;
         for (int c = 0; c < 4; ++c) {
-            s[c] = 0.5 * t->mu_c[(size_t)c * Ns + k];
-            s[4 + c] = t->lam_c[(size_t)c * Ns + k];
+            s[c] = -0.5 * crf::kLog2e * t->mu_c[(size_t)c * Ns + k];
+            s[4 + c] = crf::kLog2e * t->lam_c[(size_t)c * Ns + k];
             dd[4 * (size_t)k + c] = t->D_c[(size_t)c * npair + pair_index(k, k)];
         }
-        s[8] = 1.0 / std::sqrt(std::sqrt(t->W[k]));
+        s[8] = std::sqrt(std::sqrt(t->W[k]));
         s[9] = std::sqrt(t->W[k]);
         s[10] = 1.0 / t->W[k];
     }

@@ -175,29 +175,38 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
     double invW[PPL], sum_a[PPL], sum_h[PPL];
 #pragma unroll
     for (int u = 0; u < PPL; ++u) invW[u] = sum_a[u] = sum_h[u] = 0.0;
-    for (int k = warp; k < NsP; k += W) {
-        double z[PPL], r[PPL];
+    // (groups of G species: the G row loads are in flight together)
+    constexpr int G = 8 / PPL;
+    for (int k0 = warp; k0 < NsP; k0 += G * W) {
+        double y[G][PPL];
 #pragma unroll
-        for (int u = 0; u < PPL; ++u) z[u] = r[u] = 0.0;
-        if (k < Ns) {
-            const double *sp = tp.sp + 12 * k;
-            double y[PPL];
-            load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y);
+        for (int g = 0; g < G; ++g) {
+            const int k = k0 + g * W;
+            if (k < Ns) {
+                load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y[g]);
+            } else {
 #pragma unroll
-            for (int u = 0; u < PPL; ++u) {
-                z[u] = y[u] * __ldg(sp + 10);
-                const double smu = exp(cubic4(sp, L[u]));      // sqrt(mu_k)
-                const double lam = exp(cubic4(sp + 4, L[u]));  // lambda_k
-                r[u] = 1.0 / (smu * __ldg(sp + 8));            // 1/a_k
-                invW[u] += z[u];
-                sum_a[u] = fma(z[u], lam, sum_a[u]);
-                sum_h[u] += z[u] / lam;
+                for (int u = 0; u < PPL; ++u) y[g][u] = 0.0;
             }
         }
 #pragma unroll
-        for (int u = 0; u < PPL; ++u) {
-            sZ[ROW(k, u) + lane] = z[u];
-            sS[ROW(k, u) + lane] = r[u];
+        for (int g = 0; g < G; ++g) {
+            const int k = k0 + g * W;
+            if (k < NsP) {
+                const double *sp = tp.sp + 12 * k;  // padded rows are all zero: z = 0, r = 0
+                const double rW = __ldg(sp + 10), w4 = __ldg(sp + 8);
+#pragma unroll
+                for (int u = 0; u < PPL; ++u) {
+                    const double z = y[g][u] * rW;
+                    const double r = exp2_poly9(cubic4(sp, L[u])) * w4;   // 1/a_k = W_k^(1/4) / sqrt(mu_k)
+                    const double lam = exp2_poly9(cubic4(sp + 4, L[u]));  // lambda_k
+                    invW[u] += z;
+                    sum_a[u] = fma(z, lam, sum_a[u]);
+                    sum_h[u] = fma(z, crf::rcp_newton(lam), sum_h[u]);
+                    sZ[ROW(k, u) + lane] = z;
+                    sS[ROW(k, u) + lane] = r;
+                }
+            }
         }
     }
 #pragma unroll
@@ -230,29 +239,35 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
             }
             const int ld = 8 * nJ;  // row length of the slab
             const double *cw = reinterpret_cast<const double *>(sStage + (size_t)(s & 1) * tp.stage_bytes) + warp * 8 * ld;
-            for (int jj = 0; jj < nJ; ++jj) {
+            // four columns at a time: 12 right-hand-side values in registers leave room for the compiler to
+            // keep several coefficient loads in flight
+            for (int j4 = 0; j4 < 2 * nJ; ++j4) {
 #pragma unroll
                 for (int u = 0; u < PPL; ++u) {
-                    double u0[8], u1[8], u2[8];
+                    double u0[4], u1[4], u2[4];
 #pragma unroll
-                    for (int b = 0; b < 8; ++b) {
-                        u0[b] = sZl[ROW(8 * (J0 + jj) + b, u)];
-                        const double r = sSl[ROW(8 * (J0 + jj) + b, u)];
+                    for (int b = 0; b < 4; ++b) {
+                        u0[b] = sZl[ROW(8 * J0 + 4 * j4 + b, u)];
+                        const double r = sSl[ROW(8 * J0 + 4 * j4 + b, u)];
                         u1[b] = u0[b] * r;
                         u2[b] = u1[b] * r;
                     }
 #pragma unroll
                     for (int a = 0; a < 8; ++a) {
-#pragma unroll
-                        for (int b = 0; b < 8; b += 2) {
-                            const double2 cc = *reinterpret_cast<const double2 *>(cw + a * ld + 8 * jj + b);
-                            A[u][a] = fma(cc.x, u0[b], A[u][a]);
-                            B[u][a] = fma(cc.x, u1[b], B[u][a]);
-                            C[u][a] = fma(cc.x, u2[b], C[u][a]);
-                            A[u][a] = fma(cc.y, u0[b + 1], A[u][a]);
-                            B[u][a] = fma(cc.y, u1[b + 1], B[u][a]);
-                            C[u][a] = fma(cc.y, u2[b + 1], C[u][a]);
-                        }
+                        const double2 c01 = *reinterpret_cast<const double2 *>(cw + a * ld + 4 * j4);
+                        const double2 c23 = *reinterpret_cast<const double2 *>(cw + a * ld + 4 * j4 + 2);
+                        A[u][a] = fma(c01.x, u0[0], A[u][a]);
+                        B[u][a] = fma(c01.x, u1[0], B[u][a]);
+                        C[u][a] = fma(c01.x, u2[0], C[u][a]);
+                        A[u][a] = fma(c01.y, u0[1], A[u][a]);
+                        B[u][a] = fma(c01.y, u1[1], B[u][a]);
+                        C[u][a] = fma(c01.y, u2[1], C[u][a]);
+                        A[u][a] = fma(c23.x, u0[2], A[u][a]);
+                        B[u][a] = fma(c23.x, u1[2], B[u][a]);
+                        C[u][a] = fma(c23.x, u2[2], C[u][a]);
+                        A[u][a] = fma(c23.y, u0[3], A[u][a]);
+                        B[u][a] = fma(c23.y, u1[3], B[u][a]);
+                        C[u][a] = fma(c23.y, u2[3], C[u][a]);
                     }
                 }
             }
@@ -264,10 +279,10 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
                         const double wk = __ldg(tp.sp + 12 * k + 9);
 #pragma unroll
                         for (int u = 0; u < PPL; ++u) {
-                            const double ak = 1.0 / sSl[ROW(k, u)];
+                            const double ak = crf::rcp_newton(sSl[ROW(k, u)]);
                             const double ak2 = ak * ak;
                             const double den = fma(ak2, C[u][a], fma(ak + ak, B[u][a], A[u][a]));
-                            mu_p[u] += sZl[ROW(k, u)] * (ak2 * wk) / den;
+                            mu_p[u] = fma(sZl[ROW(k, u)] * (ak2 * wk), crf::rcp_newton(den), mu_p[u]);
                         }
                     }
                 }
@@ -331,18 +346,27 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
     double f[PPL];
 #pragma unroll
     for (int u = 0; u < PPL; ++u) f[u] = m.p_ref / (CRF_R_GAS * Ti[u]);
-    for (int k = warp; k < Ns; k += W) {
-        double y[PPL], v[PPL];
-        load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y);
+    for (int k0 = warp; k0 < Ns; k0 += G * W) {
+        double y[G][PPL];
 #pragma unroll
-        for (int u = 0; u < PPL; ++u) {
-            const double s = sS[ROW(k, u) + lane];
-            if (s == 0.0)
-                v[u] = f[u] / iw[u] * exp(cubic4(tp.Ddiag + 4 * k, L[u]));
-            else
-                v[u] = f[u] * (1.0 - y[u]) / s;
+        for (int g = 0; g < G; ++g)
+            if (k0 + g * W < Ns) load_row<PPL>(Y + (int64_t)(k0 + g * W) * n, i0, n, vec, y[g]);
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const int k = k0 + g * W;
+            if (k < Ns) {
+                double v[PPL];
+#pragma unroll
+                for (int u = 0; u < PPL; ++u) {
+                    const double s = sS[ROW(k, u) + lane];
+                    if (s == 0.0)
+                        v[u] = f[u] / iw[u] * exp(cubic4(tp.Ddiag + 4 * k, L[u]));
+                    else
+                        v[u] = f[u] * (1.0 - y[g][u]) * crf::rcp_newton(s);
+                }
+                store_row<PPL>(rhoD + (int64_t)k * n, i0, n, vec, v);
+            }
         }
-        store_row<PPL>(rhoD + (int64_t)k * n, i0, n, vec, v);
     }
 }
 
