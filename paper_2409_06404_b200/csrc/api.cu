@@ -185,9 +185,8 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
     d.mu_c = D(omu), d.lam_c = D(olam), d.nDc = D(onD), d.wilke_c = D(owk), d.wq = D(owq);
     TransportPlan &tp = d.tp;
     tp.W = tpo.W, tp.PPL = tpo.PPL, tp.NsP = tpo.NsP, tp.nb = tpo.nb, tp.n_wilke = tpo.n_wilke, tp.n_rounds = tpo.n_rounds;
-    tp.stage_bytes = tpo.stage_bytes;
+    tp.stage_bytes = tpo.stage_bytes, tp.dbg_skip = tpo.dbg_skip;
     tp.rounds = reinterpret_cast<const int4 *>(base + tpo.rounds);
-    tp.sched = reinterpret_cast<const int2 *>(base + tpo.sched);
     tp.pair_coef = base + tpo.pair_coef, tp.wilke_cP = D(tpo.wilke_cP), tp.sp = D(tpo.sp), tp.Ddiag = D(tpo.Ddiag);
     RatesPlan &rp = d.rp;
     rp.W = rpo.W, rp.Rc = rpo.Rc, rp.n_chunks = rpo.n_chunks;

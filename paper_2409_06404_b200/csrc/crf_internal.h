@@ -15,15 +15,18 @@ struct TransportPlan {
     int W;         // warps per block (1, 2, 4 or 8); 0 = no plan (generic kernel)
     int PPL;       // points per lane (1 or 2)
     int NsP, nb;   // padded species count (multiple of 8) and number of 8-blocks
+    int dbg_skip;  // tuning only (CRF_TRANSPORT_SKIP): bit 0 skips the Wilke arithmetic, bit 1 the pair arithmetic
     int n_wilke;   // stage blocks of the Wilke phase (they come first in `rounds`)
     int n_rounds;  // stage blocks (rounds) of the pair phase
     int stage_bytes;          // largest stage block (multiple of 16)
-    const int4 *rounds;       // [n_wilke + n_rounds]: x = byte offset of the block in pair_coef, y = its bytes;
+    const int4 *rounds;       // [n_wilke + n_rounds] stage blocks: x = byte offset in pair_coef, y = bytes;
                               //   Wilke blocks: z = first column block | pass << 8 | first panel << 16 |
-                              //   last panel << 17, w = column blocks nJ; layout [W][8 rows][8 nJ] of c_kj
-    const int2 *sched;        // [n_rounds][W]: x = kind | jb << 8 | kb << 16 (kind 0 idle, 1 off-diagonal,
-                              //   2 diagonal), y = byte offset of the tile's coefficients inside the round block
-    const unsigned char *pair_coef;  // per pair (c0,c1,c2,c3) of -log2(e) * ln D_jk fit; 0 for padding
+                              //   last panel << 17, w = column blocks nJ
+    const unsigned char *pair_coef;  // the stage blocks.  Block = header {int4 descriptor of the next block,
+                              //   int2 sched[W] (pair rounds): x = kind | jb << 8 | kb << 16 (kind 0 idle, 1 off-diagonal,
+                              //   2 diagonal), y = byte offset of the tile's coefficients in the block}, padded to 16 bytes;
+                              //   payload: Wilke [W][8 rows][8 nJ] of c_kj, or per pair (c0,c1,c2,c3) of the
+                              //   -log2(e) ln D_jk fit (0 for padding)
     const double *wilke_cP;   // [NsP][NsP] c_kj = 1/sqrt(8 (1 + W_k/W_j)), 0 in padded rows/columns
     const double *sp;         // [NsP][12]: 0-3 -log2(e) ln(mu_k)/2 cubic, 4-7 log2(e) ln(lambda_k) cubic, 8 W^1/4, 9 W^1/2,
                               //   10 1/W (0 for padding), 11 unused

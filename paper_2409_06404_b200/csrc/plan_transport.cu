@@ -72,6 +72,7 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
     int PPL = env_int("CRF_TRANSPORT_PPL", 1);
     if (PPL != 1 && PPL != 2) PPL = 1;
     o.W = W, o.PPL = PPL, o.NsP = NsP, o.nb = nb;
+    o.dbg_skip = env_int("CRF_TRANSPORT_SKIP", 0);
 
     const int npair = Ns * (Ns + 1) / 2;
     auto pair_index = [&](int j, int k) {
@@ -82,46 +83,56 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
         for (int c = 0; c < 4; ++c)
             dst.push_back(j < Ns && k < Ns ? -crf::kLog2e * t->D_c[(size_t)c * npair + pair_index(j, k)] : 0.0);
     };
-    std::vector<int2> sched;
+    // Stage blocks (Wilke panels first, then the pair rounds).  Every block starts with a header of
+    // hdr = 16 + 8 W (rounded up to 16) bytes: int4 descriptor of the NEXT block {byte offset in pair_coef, bytes,
+    // flags, nJ} and, in pair rounds, int2 sched[W] {kind | jb << 8 | kb << 16, byte offset of the tile's
+    // coefficients from the block start}: the kernel's loops read no descriptor from global memory.
+    const size_t hdr_d = (16 + 8 * (size_t)W + 15) / 16 * 2;  // header size in doubles
     std::vector<int4> rdesc;
     std::vector<double> coef;
     size_t stage_bytes = 16;
+    auto put_i = [&](size_t byte_off, int v) { std::memcpy(reinterpret_cast<unsigned char *>(coef.data()) + byte_off, &v, 4); };
+    auto close_block = [&](size_t start, int flags, int nJ) {
+        if (coef.size() & 1) coef.push_back(0.0);
+        rdesc.push_back(make_int4((int)(8 * start), (int)(8 * (coef.size() - start)), flags, nJ));
+        stage_bytes = std::max(stage_bytes, 8 * (coef.size() - start));
+    };
     // Wilke stage blocks: pass p covers the row blocks p W .. p W + W - 1 (one per warp), a panel covers up to
-    // kPanel column blocks; block layout [W][8 rows][8 nJ columns] of c_kj (0 in padded rows/columns)
+    // kPanel column blocks; payload [W][8 rows][8 nJ columns] of c_kj (0 in padded rows/columns)
     const int kPanel = 3, npass = (nb + W - 1) / W;
     for (int ps = 0; ps < npass; ++ps)
         for (int J0 = 0; J0 < nb; J0 += kPanel) {
             const int nJ = std::min(kPanel, nb - J0);
             const size_t start = coef.size();
+            coef.resize(start + hdr_d, 0.0);
             for (int w = 0; w < W; ++w)
                 for (int a = 0; a < 8; ++a)
                     for (int c = 0; c < 8 * nJ; ++c) {
                         const int k = 8 * (ps * W + w) + a, j = 8 * J0 + c;
                         coef.push_back(k < Ns && j < Ns ? 1.0 / std::sqrt(8.0 * (1.0 + t->W[k] / t->W[j])) : 0.0);
                     }
-            const int flags = J0 | ps << 8 | (J0 == 0) << 16 | (J0 + nJ == nb) << 17;
-            rdesc.push_back(make_int4((int)(8 * start), (int)(8 * (coef.size() - start)), flags, nJ));
-            stage_bytes = std::max(stage_bytes, 8 * (coef.size() - start));
+            close_block(start, J0 | ps << 8 | (J0 == 0) << 16 | (J0 + nJ == nb) << 17, nJ);
         }
     o.n_wilke = (int)rdesc.size();
     for (auto &rd : schedule_rounds(nb, W)) {
         const size_t start = coef.size();
-        for (int w = 0; w < W; ++w) {
-            if (w >= (int)rd.size()) {
-                sched.push_back(make_int2(0, 0));
-                continue;
-            }
+        coef.resize(start + hdr_d, 0.0);
+        for (int w = 0; w < (int)rd.size(); ++w) {
             const Tile &tl = rd[w];
-            sched.push_back(make_int2(tl.kind | tl.jb << 8 | tl.kb << 16, (int)(8 * (coef.size() - start))));
+            put_i(8 * start + 16 + 8 * (size_t)w, tl.kind | tl.jb << 8 | tl.kb << 16);
+            put_i(8 * start + 16 + 8 * (size_t)w + 4, (int)(8 * (coef.size() - start)));
             for (int a = 0; a < 8; ++a)
                 for (int c = tl.kind == 1 ? 0 : a + 1; c < 8; ++c) put_pair(coef, 8 * tl.jb + a, 8 * tl.kb + c);
         }
-        if (coef.size() & 1) coef.push_back(0.0);
-        rdesc.push_back(make_int4((int)(8 * start), (int)(8 * (coef.size() - start)), 0, 0));
-        stage_bytes = std::max(stage_bytes, 8 * (coef.size() - start));
+        close_block(start, 0, 0);
     }
     o.n_rounds = (int)rdesc.size() - o.n_wilke;
     o.stage_bytes = (int)stage_bytes;
+    for (size_t i = 0; i + 1 < rdesc.size(); ++i) {
+        const int4 nx = rdesc[i + 1];
+        put_i((size_t)rdesc[i].x + 0, nx.x), put_i((size_t)rdesc[i].x + 4, nx.y);
+        put_i((size_t)rdesc[i].x + 8, nx.z), put_i((size_t)rdesc[i].x + 12, nx.w);
+    }
 
     std::vector<double> cP((size_t)NsP * NsP, 0.0), sp((size_t)NsP * 12, 0.0), dd((size_t)Ns * 4);
     for (int k = 0; k < Ns; ++k) {
@@ -136,6 +147,6 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
         s[9] = std::sqrt(t->W[k]);
         s[10] = 1.0 / t->W[k];
     }
-    o.rounds = b.add(rdesc), o.sched = b.add(sched), o.pair_coef = b.add(coef), o.wilke_cP = b.add(cP), o.sp = b.add(sp), o.Ddiag = b.add(dd);
+    o.rounds = b.add(rdesc), o.pair_coef = b.add(coef), o.wilke_cP = b.add(cP), o.sp = b.add(sp), o.Ddiag = b.add(dd);
     return o;
 }

@@ -28,6 +28,9 @@
 namespace {
 
 using crf::exp2_poly9;
+using crf::exp2_tab16;
+
+__constant__ double kExp2Tab16[16] = CRF_EXP2_TAB16;
 
 __device__ __forceinline__ double cubic4(const double *__restrict__ c, double x)
 {
@@ -42,7 +45,7 @@ __device__ __forceinline__ double cubic4(const double *__restrict__ c, double x)
 // off-diagonal tile: species blocks jb < kb, 64 pairs; cf: the tile's coefficients in shared memory
 template <int PPL>
 __device__ __forceinline__ void tile_offdiag(const double2 *cf, const double (&L)[PPL], const double *sZl, double *sSl,
-                                             int jb, int kb)
+                                             int jb, int kb, const double *tab)
 {
     double zj[PPL][8], zk[PPL][8], sj[PPL][8], sk[PPL][8];
 #pragma unroll
@@ -61,7 +64,7 @@ __device__ __forceinline__ void tile_offdiag(const double2 *cf, const double (&L
             const double2 lo = cf[2 * (8 * a + b)], hi = cf[2 * (8 * a + b) + 1];
 #pragma unroll
             for (int u = 0; u < PPL; ++u) {
-                const double e = exp2_poly9(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x));
+                const double e = exp2_tab16(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x), tab);
                 sj[u][a] = fma(zk[u][b], e, sj[u][a]);
                 sk[u][b] = fma(zj[u][a], e, sk[u][b]);
             }
@@ -78,7 +81,8 @@ __device__ __forceinline__ void tile_offdiag(const double2 *cf, const double (&L
 
 // diagonal tile: pairs a < b inside block jb, 28 pairs
 template <int PPL>
-__device__ __forceinline__ void tile_diag(const double2 *cf, const double (&L)[PPL], const double *sZl, double *sSl, int jb)
+__device__ __forceinline__ void tile_diag(const double2 *cf, const double (&L)[PPL], const double *sZl, double *sSl, int jb,
+                                          const double *tab)
 {
     double z[PPL][8], s[PPL][8];
 #pragma unroll
@@ -96,7 +100,7 @@ __device__ __forceinline__ void tile_diag(const double2 *cf, const double (&L)[P
             const double2 lo = cf[2 * q], hi = cf[2 * q + 1];
 #pragma unroll
             for (int u = 0; u < PPL; ++u) {
-                const double e = exp2_poly9(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x));
+                const double e = exp2_tab16(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x), tab);
                 s[u][a] = fma(z[u][b], e, s[u][a]);
                 s[u][b] = fma(z[u][a], e, s[u][b]);
             }
@@ -148,6 +152,8 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
                            double *__restrict__ mu, double *__restrict__ lambda, double *__restrict__ rhoD)
 {
     extern __shared__ double2 sm2[];
+    __shared__ double sTab[16];
+    if (threadIdx.x < 16) sTab[threadIdx.x] = kExp2Tab16[threadIdx.x];
     double *sm = reinterpret_cast<double *>(sm2);
     const TransportPlan &tp = m.tp;
     const int Ns = m.Ns, NsP = tp.NsP, nb = tp.nb;
@@ -159,10 +165,9 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
     const double *sZl = sZ + lane;
     double *sSl = sS + lane;
 
-    {
-        const int4 r0 = __ldg(tp.rounds);
-        stage_async(sStage, tp.pair_coef + r0.x, r0.y, threadIdx.x, 32 * W);
-    }
+    int4 cur = __ldg(tp.rounds);  // descriptor of the block being staged / used; later ones come with the blocks
+    stage_async(sStage, tp.pair_coef + cur.x, cur.y, threadIdx.x, 32 * W);
+    constexpr int HDR = (16 + 8 * W + 15) / 16 * 16;
 
     const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * PPL;
     const bool vec = (n & 1) == 0;
@@ -227,10 +232,12 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
         for (int s = 0; s < nwk; ++s) {
             stage_wait();
             __syncthreads();  // block s has landed; everyone is done with block s - 1
-            const int4 ds = __ldg(tp.rounds + s), d1 = __ldg(tp.rounds + s + 1);
-            stage_async(sStage + (size_t)((s + 1) & 1) * tp.stage_bytes, tp.pair_coef + d1.x, d1.y, threadIdx.x, 32 * W);
+            const unsigned char *blk = sStage + (size_t)(s & 1) * tp.stage_bytes;
+            const int4 ds = cur;
+            cur = *reinterpret_cast<const int4 *>(blk);
+            stage_async(sStage + (size_t)((s + 1) & 1) * tp.stage_bytes, tp.pair_coef + cur.x, cur.y, threadIdx.x, 32 * W);
             const int J0 = ds.z & 0xff, I = ((ds.z >> 8) & 0xff) * W + warp, nJ = ds.w;
-            if (I >= nb) continue;
+            if (I >= nb || (tp.dbg_skip & 1)) continue;
             if (ds.z & (1 << 16)) {
 #pragma unroll
                 for (int u = 0; u < PPL; ++u)
@@ -238,7 +245,7 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
                     for (int a = 0; a < 8; ++a) A[u][a] = B[u][a] = C[u][a] = 0.0;
             }
             const int ld = 8 * nJ;  // row length of the slab
-            const double *cw = reinterpret_cast<const double *>(sStage + (size_t)(s & 1) * tp.stage_bytes) + warp * 8 * ld;
+            const double *cw = reinterpret_cast<const double *>(blk + HDR) + warp * 8 * ld;
             // four columns at a time: 12 right-hand-side values in registers leave room for the compiler to
             // keep several coefficient loads in flight
             for (int j4 = 0; j4 < 2 * nJ; ++j4) {
@@ -328,16 +335,17 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
     for (int rd = 0; rd < nrd; ++rd) {
         const unsigned char *blk = sStage + (size_t)((nwk + rd) & 1) * tp.stage_bytes;
         if (rd + 1 < nrd) {
-            const int4 r1 = __ldg(tp.rounds + nwk + rd + 1);
+            const int4 r1 = *reinterpret_cast<const int4 *>(blk);
             stage_async(sStage + (size_t)((nwk + rd + 1) & 1) * tp.stage_bytes, tp.pair_coef + r1.x, r1.y, threadIdx.x, 32 * W);
         }
-        const int2 d = __ldg(tp.sched + rd * W + warp);
+        const int2 d = *reinterpret_cast<const int2 *>(blk + 16 + 8 * warp);
         const int kind = d.x & 0xff, jb = (d.x >> 8) & 0xff, kb = (d.x >> 16) & 0xff;
         const double2 *cf = reinterpret_cast<const double2 *>(blk + d.y);
-        if (kind == 1)
-            tile_offdiag<PPL>(cf, L, sZl, sSl, jb, kb);
+        if (tp.dbg_skip & 2) {
+        } else if (kind == 1)
+            tile_offdiag<PPL>(cf, L, sZl, sSl, jb, kb, sTab);
         else if (kind == 2)
-            tile_diag<PPL>(cf, L, sZl, sSl, jb);
+            tile_diag<PPL>(cf, L, sZl, sSl, jb, sTab);
         stage_wait();
         __syncthreads();
     }
