@@ -108,16 +108,18 @@ std::vector<unsigned char> chunk_block(const Builder &B, const Chunk &ch, int PP
         put(v, o_slot + slot_row * w, (unsigned)v.size());
         for (int sl = 0; sl < maxown; ++sl) {
             const int k = w + W * sl;
+            int cnt_slot = 0;
             for (int rl = 0; rl < cnt && k < Ns; ++rl) {
                 const int r = ch.reactions[rl];
                 int nu = 0;
                 for (int s = 0; s < 3; ++s) nu += (B.slot(t->prod, s, r) == k) - (B.slot(t->reac, s, r) == k);
-                if (nu != 0) append16((double)nu, (unsigned)rl * qrow);
+                if (nu != 0) append16((double)nu, (unsigned)rl * qrow), ++cnt_slot;
             }
+            if (cnt_slot & 1) append16(0.0, 0u);  // the entry loop takes two entries per trip
             put(v, o_slot + slot_row * w + 16 + 4 * (size_t)sl, (unsigned)v.size());
         }
     }
-    append16(0.0, 0u);  // the entry loop reads one entry ahead
+    append16(0.0, 0u), append16(0.0, 0u);  // the entry loop reads two entries ahead
     for (int rl = 0; rl < cnt; ++rl) {
         const int r = ch.reactions[rl];
         const size_t o = 48 * (size_t)rl;
@@ -171,16 +173,18 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
     // two chunk blocks.  CRF_RATES_W / CRF_RATES_PPL / CRF_RATES_RC override (tuning).
     auto budget = [](int W) { return (size_t)233472 / (16 / W) - 1024; };
     auto state = [&](int PPL) { return (size_t)(Ns + 1) * 512 * PPL; };
-    // measured on C5 (Ns = 118): W/PPL = 16/2 11.2 ms, 8/1 13.8 ms, 16/1 14.4 ms -> large mechanisms take the
-    // whole SM as one block with two points per lane
-    const bool big = Ns > 64 && state(2) <= budget(16) * 6 / 10;
-    int PPL = env_int("CRF_RATES_PPL", Ns <= 32 || big ? 2 : 1);
+    // Measured (rates, ms): C5 W/PPL 16/2 11.0, 8/1 13.8, 16/1 14.4; C4 8/2 9.0, 16/2 10.9, 8/1 13.0, 4/2 21.0;
+    // C3 4/2 2.6, 8/2 3.0, 4/1 4.2; C2 4/2 3.4, 4/1 5.5 -> two points per lane whenever the state fits, and the
+    // fewest warps whose share of the SM's shared memory holds the state with room for the q buffer.
+    auto pick_w = [&](int ppl) {
+        for (int w = 4; w <= 16; w *= 2)
+            if (state(ppl) <= budget(w) * 6 / 10 && (Ns + w - 1) / w <= 16) return w;
+        return 0;
+    };
+    int PPL = env_int("CRF_RATES_PPL", pick_w(2) ? 2 : 1);
     if (PPL != 1 && PPL != 2) PPL = 1;
-    int W = env_int("CRF_RATES_W", big && PPL == 2 ? 16 : 0);
-    if (W != 4 && W != 8 && W != 16) {
-        W = 4;
-        while (W < 16 && (state(PPL) > budget(W) * 6 / 10 || (Ns + W - 1) / W > 16)) W *= 2;
-    }
+    int W = env_int("CRF_RATES_W", 0);
+    if (W != 4 && W != 8 && W != 16) W = pick_w(PPL) ? pick_w(PPL) : 16;
     if ((Ns + W - 1) / W > 16 || state(PPL) + 2 * W * 256 * PPL > budget(W)) return o;
 
     const int own = (Ns + W - 1) / W, maxown = own <= 4 ? 4 : (own <= 8 ? 8 : 16);

@@ -263,31 +263,42 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     double invW[PPL];
 #pragma unroll
     for (int u = 0; u < PPL; ++u) invW[u] = 0.0;
-    for (int k = warp; k < Ns; k += W) {
-        const double2 *g = reinterpret_cast<const double2 *>(rs.gco + 16 * (size_t)k);
-        const double2 l01 = __ldg(g), l23 = __ldg(g + 1), l45 = __ldg(g + 2), l6t = __ldg(g + 3);
-        const double2 h01 = __ldg(g + 4), h23 = __ldg(g + 5), h45 = __ldg(g + 6), h6w = __ldg(g + 7);
-        double y[PPL];
-        load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y);
+    // (slots in groups of 4: the four Y row loads and the coefficient loads are in flight together)
 #pragma unroll
-        for (int u = 0; u < PPL; ++u) {
-            const double Tu = c.T[u], oml = 1.0 - c.L[u];
-            double lo = fma(Tu, l45.x, l23.y);
-            lo = fma(Tu, lo, l23.x);
-            lo = fma(Tu, lo, l01.y);
-            lo = fma(Tu, lo, l6t.x);
-            lo = fma(l45.y, c.rT[u], lo);
-            lo = fma(l01.x, oml, lo);
-            double hi = fma(Tu, h45.x, h23.y);
-            hi = fma(Tu, hi, h23.x);
-            hi = fma(Tu, hi, h01.y);
-            hi = fma(Tu, hi, h6w.x);
-            hi = fma(h45.y, c.rT[u], hi);
-            hi = fma(h01.x, oml, hi);
-            const double g2 = Tu <= l6t.y ? lo : hi;
-            const double z = y[u] * h6w.y;
-            invW[u] += z;
-            *reinterpret_cast<double2 *>(sL + (size_t)k * 512 * PPL + 512 * u) = make_double2(z, exp2c(lc02[u] - g2));
+    for (int s0 = 0; s0 < MAXOWN; s0 += 4) {
+        double y[4][PPL];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int k = warp + W * (s0 + j);
+            if (k < Ns) load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int k = warp + W * (s0 + j);
+            if (k >= Ns) continue;
+            const double2 *g = reinterpret_cast<const double2 *>(rs.gco + 16 * (size_t)k);
+            const double2 l01 = __ldg(g), l23 = __ldg(g + 1), l45 = __ldg(g + 2), l6t = __ldg(g + 3);
+            const double2 h01 = __ldg(g + 4), h23 = __ldg(g + 5), h45 = __ldg(g + 6), h6w = __ldg(g + 7);
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) {
+                const double Tu = c.T[u], oml = 1.0 - c.L[u];
+                double lo = fma(Tu, l45.x, l23.y);
+                lo = fma(Tu, lo, l23.x);
+                lo = fma(Tu, lo, l01.y);
+                lo = fma(Tu, lo, l6t.x);
+                lo = fma(l45.y, c.rT[u], lo);
+                lo = fma(l01.x, oml, lo);
+                double hi = fma(Tu, h45.x, h23.y);
+                hi = fma(Tu, hi, h23.x);
+                hi = fma(Tu, hi, h01.y);
+                hi = fma(Tu, hi, h6w.x);
+                hi = fma(h45.y, c.rT[u], hi);
+                hi = fma(h01.x, oml, hi);
+                const double g2 = Tu <= l6t.y ? lo : hi;
+                const double z = y[j][u] * h6w.y;
+                invW[u] += z;
+                *reinterpret_cast<double2 *>(sL + (size_t)k * 512 * PPL + 512 * u) = make_double2(z, exp2c(lc02[u] - g2));
+            }
         }
     }
     if (warp == 0) {
@@ -340,7 +351,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
             // the warp's entries are contiguous (slot-major); slot s ends at ends[s]; one entry is read ahead
             const char *sr = blk + o_slot + SLOT_ROW * warp;
             unsigned e = *reinterpret_cast<const unsigned *>(sr);
-            uint4 en = ldsu4(blk + e);
+            uint4 en0 = ldsu4(blk + e), en1 = ldsu4(blk + e + 16);
 #pragma unroll
             for (int s4 = 0; s4 < MAXOWN; s4 += 4) {
                 const uint4 ends = ldsu4(sr + 16 + 4 * s4);
@@ -348,14 +359,21 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
                 for (int j = 0; j < 4; ++j) {
                     const int s = s4 + j;
                     const unsigned end = j == 0 ? ends.x : (j == 1 ? ends.y : (j == 2 ? ends.z : ends.w));
-                    while (e < end) {
-                        const uint4 cur = en;
-                        e += 16;
-                        en = ldsu4(blk + e);
-                        const double nu = __hiloint2double((int)cur.y, (int)cur.x);
+#pragma unroll 1
+                    while (e < end) {  // two entries per trip (lists are padded to even length)
+                        const uint4 c0 = en0, c1 = en1;
+                        e += 32;
+                        en0 = ldsu4(blk + e), en1 = ldsu4(blk + e + 16);
+                        const double nu0 = __hiloint2double((int)c0.y, (int)c0.x);
+                        const double nu1 = __hiloint2double((int)c1.y, (int)c1.x);
+                        double q0[PPL], q1[PPL];
 #pragma unroll
-                        for (int u = 0; u < PPL; ++u)
-                            om[s][u] = fma(nu, *reinterpret_cast<const double *>(sQl + cur.z + 256 * u), om[s][u]);
+                        for (int u = 0; u < PPL; ++u) {
+                            q0[u] = *reinterpret_cast<const double *>(sQl + c0.z + 256 * u);
+                            q1[u] = *reinterpret_cast<const double *>(sQl + c1.z + 256 * u);
+                        }
+#pragma unroll
+                        for (int u = 0; u < PPL; ++u) om[s][u] = fma(nu1, q1[u], fma(nu0, q0[u], om[s][u]));
                     }
                 }
             }
