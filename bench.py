@@ -104,6 +104,21 @@ def reference_arm(args):
     return 0
 
 
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on `workload`, from the committed
+    ncu --set full summary (profiles/r01_dram_traffic.csv: a measurement made under the profiler, not by this run)."""
+    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    try:
+        with open(path) as f:
+            for row in f.read().splitlines()[1:]:
+                c = row.split(",")
+                if len(c) >= 4 and c[0] == workload and c[1] == kernel:
+                    return float(c[2]) + float(c[3])
+    except OSError:
+        pass
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -287,17 +302,18 @@ def main():
                        "bound": "alu" if t_alu >= t_hbm else "hbm", "tflops": w["F"] * n / (ms * 1e-3) / 1e12,
                        "gbs": w["B"] * n / (ms * 1e-3) / 1e9, "frac_of_roofline": max(t_alu, t_hbm) / (ms * 1e-3)}
     dom = max(names, key=lambda k: kernels[k]["ms"])
+    traffic = ncu_traffic(name, dom)
     kd = kernels[dom]
     if kd["bound"] == "alu":
         roof = {"bound": "alu", "kernel": dom, "achieved": kd["tflops"], "peak": rooflines.FP64_PEAK_TFLOPS,
-                "unit": "TFLOP/s", "frac": kd["tflops"] / rooflines.FP64_PEAK_TFLOPS, "traffic": None,
+                "unit": "TFLOP/s", "frac": kd["tflops"] / rooflines.FP64_PEAK_TFLOPS, "traffic": traffic,
                 "peak_source": "148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md); FMA = 2 flops",
                 "peak_measured_dfma": 2 * fp64_inst / 1e12,
                 "frac_of_measured_dfma": kd["tflops"] / (2 * fp64_inst / 1e12) if fp64_inst else None,
                 "flops_per_point": work[dom]["F"], "fp64_instr_per_point": work[dom]["I"]}
     else:
         roof = {"bound": "hbm", "kernel": dom, "achieved": kd["gbs"], "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": kd["gbs"] / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+                "frac": kd["gbs"] / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"],
                 "bytes_per_point": work[dom]["B"]}
 
     cpu = None
