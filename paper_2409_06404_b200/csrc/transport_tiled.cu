@@ -28,9 +28,9 @@
 namespace {
 
 using crf::exp2_poly9;
-using crf::exp2_tab16;
+using crf::exp2_tab64;
 
-__constant__ double kExp2Tab16[16] = CRF_EXP2_TAB16;
+__constant__ double kExp2Tab64[64] = CRF_EXP2_TAB64;
 
 __device__ __forceinline__ double cubic4(const double *__restrict__ c, double x)
 {
@@ -64,7 +64,7 @@ __device__ __forceinline__ void tile_offdiag(const double2 *cf, const double (&L
             const double2 lo = cf[2 * (8 * a + b)], hi = cf[2 * (8 * a + b) + 1];
 #pragma unroll
             for (int u = 0; u < PPL; ++u) {
-                const double e = exp2_tab16(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x), tab);
+                const double e = exp2_tab64(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x), tab);
                 sj[u][a] = fma(zk[u][b], e, sj[u][a]);
                 sk[u][b] = fma(zj[u][a], e, sk[u][b]);
             }
@@ -100,7 +100,7 @@ __device__ __forceinline__ void tile_diag(const double2 *cf, const double (&L)[P
             const double2 lo = cf[2 * q], hi = cf[2 * q + 1];
 #pragma unroll
             for (int u = 0; u < PPL; ++u) {
-                const double e = exp2_tab16(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x), tab);
+                const double e = exp2_tab64(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x), tab);
                 s[u][a] = fma(z[u][b], e, s[u][a]);
                 s[u][b] = fma(z[u][a], e, s[u][b]);
             }
@@ -152,8 +152,8 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
                            double *__restrict__ mu, double *__restrict__ lambda, double *__restrict__ rhoD)
 {
     extern __shared__ double2 sm2[];
-    __shared__ double sTab[16];
-    if (threadIdx.x < 16) sTab[threadIdx.x] = kExp2Tab16[threadIdx.x];
+    __shared__ double sTab[64];
+    for (int i = threadIdx.x; i < 64; i += 32 * W) sTab[i] = kExp2Tab64[i];
     double *sm = reinterpret_cast<double *>(sm2);
     const TransportPlan &tp = m.tp;
     const int Ns = m.Ns, NsP = tp.NsP, nb = tp.nb;
