@@ -202,3 +202,28 @@ def test_step_host_matches_device_calls(binding, oracle_mod):
 def test_fp64_probe(binding):
     r = binding.fp64_probe(2048)
     assert 1e12 < r < 4e13, r  # B200: 148 SM x 64 lanes x ~1.9 GHz = 1.8e13 FP64 instr/s nominal
+
+
+PLAN_OVERRIDES = [
+    {"CRF_TRANSPORT_PPL": "2"},                        # two points per lane in the tiled transport kernel
+    {"CRF_TRANSPORT_W": "4"},                          # rounds split over fewer warps than tiles
+    {"CRF_TRANSPORT_W": "1", "CRF_TRANSPORT_PPL": "2"},
+    {"CRF_RATES_W": "8", "CRF_RATES_PPL": "1"},
+    {"CRF_RATES_W": "4", "CRF_RATES_PPL": "2", "CRF_RATES_RC": "32"},   # many small chunks
+    {"CRF_RATES_SMEM": "0"},                           # the staged fallback kernel
+]
+
+
+@pytest.mark.parametrize("env", PLAN_OVERRIDES, ids=lambda e: ",".join(f"{k[4:]}={v}" for k, v in e.items()))
+@pytest.mark.parametrize("name", ["C3", "C4", "C5"])
+def test_plan_overrides(binding, oracle_mod, monkeypatch, name, env):
+    """The kernel plans are chosen in crf_mech_create; the CRF_* tuning overrides select the other template
+    instances (warps per point group, points per lane, chunk size, fallback kernel): each must meet the same
+    tolerances on a ragged size."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    desc = wl.make_mechanism(name)
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    n = SMALL_N[name] + 2
+    st = wl.make_state(name, n=n, total=n)
+    parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), f"{name} {env} n={n}")
