@@ -186,6 +186,7 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
     TransportPlan &tp = d.tp;
     tp.W = tpo.W, tp.PPL = tpo.PPL, tp.NsP = tpo.NsP, tp.nb = tpo.nb, tp.n_wilke = tpo.n_wilke, tp.n_rounds = tpo.n_rounds;
     tp.stage_bytes = tpo.stage_bytes, tp.dbg_skip = tpo.dbg_skip;
+    tp.small = D(tpo.small), tp.small_n = tpo.small_n;
     tp.rounds = reinterpret_cast<const int4 *>(base + tpo.rounds);
     tp.pair_coef = base + tpo.pair_coef, tp.wilke_cP = D(tpo.wilke_cP), tp.sp = D(tpo.sp), tp.Ddiag = D(tpo.Ddiag);
     RatesPlan &rp = d.rp;

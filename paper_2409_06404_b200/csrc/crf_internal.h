@@ -31,6 +31,10 @@ struct TransportPlan {
     const double *sp;         // [NsP][12]: 0-3 -log2(e) ln(mu_k)/2 cubic, 4-7 log2(e) ln(lambda_k) cubic, 8 W^1/4, 9 W^1/2,
                               //   10 1/W (0 for padding), 11 unused
     const double *Ddiag;      // [Ns][4] ln D_kk cubic (pure-species guard)
+    // mechanisms with Ns <= 16 (W = 0): one table for transport_small.cu, small_n doubles:
+    //   sp [Ns][12] as above | Ddiag [Ns][4] | c_kj [Ns][Ns] (+ pad to even) | pair fits [Ns(Ns-1)/2][4], j < k lexicographic, as pair_coef
+    const double *small;
+    int small_n;
 };
 
 // Plan of the staged crf_production_rates kernel (rates_staged.cu).

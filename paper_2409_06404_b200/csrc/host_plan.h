@@ -24,7 +24,8 @@ struct BlockBuilder {
 // Offsets (into the block) of what a plan points to; resolved to device pointers after the upload.
 struct TransportPlanOffsets {
     int dbg_skip = 0, W = 0, PPL = 0, NsP = 0, nb = 0, n_wilke = 0, n_rounds = 0, stage_bytes = 0;
-    size_t rounds = 0, pair_coef = 0, wilke_cP = 0, sp = 0, Ddiag = 0;
+    int small_n = 0;
+    size_t small = 0, rounds = 0, pair_coef = 0, wilke_cP = 0, sp = 0, Ddiag = 0;
 };
 struct RatesPlanOffsets {
     int W = 0, Rc = 0, n_chunks = 0;

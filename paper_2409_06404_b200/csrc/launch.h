@@ -14,6 +14,8 @@ cudaError_t launch_transport(const DevTables &m, const double *T, const double *
                              double *mu, double *lambda, double *rhoD, cudaStream_t st);
 cudaError_t launch_transport_tiled(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu,
                                    double *lambda, double *rhoD, cudaStream_t st);
+cudaError_t launch_transport_small(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu,
+                                   double *lambda, double *rhoD, cudaStream_t st);
 cudaError_t launch_rates_staged(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                                 double *omega, double *qdot, cudaStream_t st);
 cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,

@@ -58,7 +58,32 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
 {
     TransportPlanOffsets o;
     const int Ns = t->Ns;
-    if (Ns < 17) return o;  // small mechanisms: generic kernel (a register-resident variant is the plan)
+    if (Ns < 17) {  // small mechanisms: the register-resident kernel (transport_small.cu), one flat table
+        if (Ns < 2 || env_int("CRF_TRANSPORT_SMALL", 1) == 0) return o;  // generic kernel
+        const int npair = Ns * (Ns + 1) / 2;
+        auto pidx = [&](int j, int k) { return j * Ns - (j * (j - 1)) / 2 + (k - j); };  // j <= k
+        std::vector<double> tb;
+        for (int k = 0; k < Ns; ++k) {
+            double s[12] = {0};
+            for (int c = 0; c < 4; ++c) {
+                s[c] = -0.5 * crf::kLog2e * t->mu_c[(size_t)c * Ns + k];
+                s[4 + c] = crf::kLog2e * t->lam_c[(size_t)c * Ns + k];
+            }
+            s[8] = std::sqrt(std::sqrt(t->W[k])), s[9] = std::sqrt(t->W[k]), s[10] = 1.0 / t->W[k];
+            tb.insert(tb.end(), s, s + 12);
+        }
+        for (int k = 0; k < Ns; ++k)
+            for (int c = 0; c < 4; ++c) tb.push_back(t->D_c[(size_t)c * npair + pidx(k, k)]);
+        for (int k = 0; k < Ns; ++k)
+            for (int j = 0; j < Ns; ++j) tb.push_back(1.0 / std::sqrt(8.0 * (1.0 + t->W[k] / t->W[j])));
+        if (tb.size() & 1) tb.push_back(0.0);  // pair fits are read as double2
+        for (int j = 0; j < Ns; ++j)
+            for (int k = j + 1; k < Ns; ++k)
+                for (int c = 0; c < 4; ++c) tb.push_back(-crf::kLog2e * t->D_c[(size_t)c * npair + pidx(j, k)]);
+        o.small_n = (int)tb.size();
+        o.small = b.add(tb);
+        return o;
+    }
     const int nb = (Ns + 7) / 8, NsP = 8 * nb;
     // warps per point group: one per tile of a round-robin round (nb odd: (nb+1)/2, nb even: nb/2), at most 8;
     // points per lane: 1 (16 warps per SM at 128 registers) or 2 (8 warps per SM, every coefficient load

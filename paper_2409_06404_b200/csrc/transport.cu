@@ -112,6 +112,7 @@ cudaError_t launch_transport(const DevTables &m, const double *T, const double *
 {
     (void)p;
     if (m.tp.W > 0) return launch_transport_tiled(m, T, Y, n, mu, lambda, rhoD, st);
+    if (m.tp.small_n > 0) return launch_transport_small(m, T, Y, n, mu, lambda, rhoD, st);
     const size_t per_thread = sizeof(double) * 4 * (size_t)m.Ns;
     const size_t budget = 100 * 1024;
     if (per_thread * 128 <= budget) return launch_b<128>(m, T, Y, n, mu, lambda, rhoD, st);
