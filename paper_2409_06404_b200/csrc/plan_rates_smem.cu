@@ -168,6 +168,23 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
         if (B.generic(r)) return o;  // a third body next to three explicit reactants: staged kernel
     if (!product_form_in_range(B)) return o;
 
+    std::vector<Chunk> chunks;
+    std::vector<std::vector<unsigned char>> blocks;
+    size_t stage_bytes = 0;
+    // Small mechanisms: one THREAD per point (rates_thread_kernel in rates_smem.cu), 128 points per block, the (C, d)
+    // state and omega as per-thread columns in shared memory (row stride 128 x 16 bytes = the layout of "4 points
+    // per lane"), all chunk blocks resident at once.  Marked W = 1, PPL = 4; stage_bytes = all blocks.
+    // Opt-in (CRF_RATES_THREAD=1): measured no faster than the warp-group kernel (C2 3.4 vs 3.4 ms, C3 3.2 vs 2.6 ms):
+    // fewer instructions per point, but the per-thread dependent shared-memory chains are not hidden.
+    if (Ns <= 24 && env_int("CRF_RATES_THREAD", 0) != 0 && env_int("CRF_RATES_W", 0) == 0) {
+        chunks = make_chunks(B, Nr);
+        for (const Chunk &ch : chunks) {
+            blocks.push_back(chunk_block(B, ch, 4, 1, 4));
+            stage_bytes += (blocks.back().size() + 15) & ~size_t(15);
+        }
+        if (stage_bytes <= 24 * 1024) o.W = 1, o.PPL = 4, o.maxown = 4, o.Rc = 0;
+    }
+    if (o.W == 0) {
     // warps per point group W and points per lane PPL: 16 warps per SM, so a block may use 1/(16/W) of the
     // SM's shared memory; the (C, d) state of its 32 PPL points should leave room for the q buffer and the
     // two chunk blocks.  CRF_RATES_W / CRF_RATES_PPL / CRF_RATES_RC override (tuning).
@@ -190,9 +207,6 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
     const int own = (Ns + W - 1) / W, maxown = own <= 4 ? 4 : (own <= 8 ? 8 : 16);
     const int step = 2 * W;
     int Rc = env_int("CRF_RATES_RC", 0);
-    std::vector<Chunk> chunks;
-    std::vector<std::vector<unsigned char>> blocks;
-    size_t stage_bytes = 0;
     for (int cand = Rc > 0 ? (Rc + step - 1) / step * step : std::min(256, (Nr + step - 1) / step * step);
          cand >= step; cand -= step) {
         chunks = make_chunks(B, cand);
@@ -206,7 +220,9 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
         if (state(PPL) + (size_t)cand * 256 * PPL + 2 * stage_bytes <= budget(W)) break;
         if (cand == step) return o;  // does not fit at all
     }
-    o.W = W, o.PPL = PPL, o.maxown = maxown, o.Rc = Rc, o.n_chunks = (int)chunks.size(), o.stage_bytes = (int)stage_bytes;
+    o.W = W, o.PPL = PPL, o.maxown = maxown, o.Rc = Rc;
+    }
+    o.n_chunks = (int)chunks.size(), o.stage_bytes = (int)stage_bytes;
 
     std::vector<int4> cdesc;
     std::vector<unsigned char> stage;

@@ -453,6 +453,148 @@ cudaError_t launch_wp(const DevTables &m, const double *T, const double *p, cons
     return cudaErrorInvalidValue;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Small mechanisms (plan W = 1, PPL = 4): one THREAD per point, 128 points per block.  The (C, d) state and the
+// omega accumulators are per-thread columns in shared memory (row stride 128 x 16 and 128 x 8 bytes), every chunk
+// block is resident, each thread walks all reactions and scatters q into its own omega column: no incidence
+// lists, no q buffer and no barrier after the tables have landed; the SM holds 12-28 warps.
+constexpr int RT_B = 128;
+
+__device__ __forceinline__ void scatter_q(char *om, const char *rec, double q, bool generic)
+{
+    const uint4 S = ldsu4(rec + 32);  // state row offsets (stride 2048) -> omega rows (stride 1024)
+    *reinterpret_cast<double *>(om + (S.x >> 1)) -= q;
+    *reinterpret_cast<double *>(om + (S.y >> 1)) -= q;
+    *reinterpret_cast<double *>(om + (S.z >> 1)) += q;
+    *reinterpret_cast<double *>(om + (S.w >> 1)) += q;
+    if (generic) {
+        const uint2 X = *reinterpret_cast<const uint2 *>(rec + 24);
+        *reinterpret_cast<double *>(om + (X.x >> 1)) -= q;
+        *reinterpret_cast<double *>(om + (X.y >> 1)) += q;
+    }
+}
+
+template <int KIND, bool GENERIC>
+__device__ __forceinline__ void thread_chunk(const char *blk, int count, int o_troe, const char *sL, char *om, const Ctx<1> &c)
+{
+    constexpr int NR = 4;  // independent reactions per trip
+    int rl = 0;
+    for (; rl + NR - 1 < count; rl += NR) {
+        double q[NR][1];
+#pragma unroll
+        for (int v = 0; v < NR; ++v)
+            reaction_q<KIND, GENERIC, 1>(blk, blk + 48 * (rl + v), blk + o_troe + 64 * (rl + v), sL, c, q[v]);
+#pragma unroll
+        for (int v = 0; v < NR; ++v) scatter_q(om, blk + 48 * (rl + v), q[v][0], GENERIC);
+    }
+    for (; rl < count; ++rl) {
+        double q0[1];
+        reaction_q<KIND, GENERIC, 1>(blk, blk + 48 * rl, blk + o_troe + 64 * rl, sL, c, q0);
+        scatter_q(om, blk + 48 * rl, q0[0], GENERIC);
+    }
+}
+
+__global__ void __launch_bounds__(RT_B) rates_thread_kernel(DevTables m, const double *__restrict__ T,
+                                                            const double *__restrict__ p, const double *__restrict__ Y,
+                                                            int64_t n, double *__restrict__ omega, double *__restrict__ qdot)
+{
+    extern __shared__ double2 sm2[];
+    const RatesSmemPlan &rs = m.rs;
+    const int Ns = m.Ns, tid = threadIdx.x;
+    char *sCD = reinterpret_cast<char *>(sm2);        // [Ns + 1][128] (C_k, d_k); row Ns = (1, 1)
+    char *sOm = sCD + (size_t)(Ns + 1) * 2048;        // [Ns + 1][128] omega_k; row Ns collects the empty slots
+    char *sTab = sOm + (size_t)(Ns + 1) * 1024;       // the chunk blocks
+    for (int o = tid * 16; o < rs.stage_bytes; o += RT_B * 16)
+        *reinterpret_cast<uint4 *>(sTab + o) = __ldg(reinterpret_cast<const uint4 *>(rs.stage + o));
+    char *sL = sCD + tid * 16, *om = sOm + tid * 8;
+
+    const int64_t i = (int64_t)blockIdx.x * RT_B + tid;
+    const int64_t ic = i < n ? i : n - 1;  // threads past the end recompute the last point and store nothing
+    Ctx<1> c;
+    c.T[0] = T[ic];
+    const double pi = p[ic], Tu = c.T[0];
+    c.L[0] = log(Tu);
+    c.rT[0] = 1.0 / Tu;
+    const double lc02 = crf::kLog2e * (log(m.p_ref / CRF_R_GAS) - c.L[0]);
+    c.Csum[0] = pi * c.rT[0] * (1.0 / CRF_R_GAS);
+    const double oml = 1.0 - c.L[0];
+
+    double invW = 0.0;
+    for (int k = 0; k < Ns; ++k) {
+        const double2 *g = reinterpret_cast<const double2 *>(rs.gco + 16 * (size_t)k);
+        const double2 l01 = __ldg(g), l23 = __ldg(g + 1), l45 = __ldg(g + 2), l6t = __ldg(g + 3);
+        const double2 h01 = __ldg(g + 4), h23 = __ldg(g + 5), h45 = __ldg(g + 6), h6w = __ldg(g + 7);
+        const double y = Y[(int64_t)k * n + ic];
+        double lo = fma(Tu, l45.x, l23.y);
+        lo = fma(Tu, lo, l23.x);
+        lo = fma(Tu, lo, l01.y);
+        lo = fma(Tu, lo, l6t.x);
+        lo = fma(l45.y, c.rT[0], lo);
+        lo = fma(l01.x, oml, lo);
+        double hi = fma(Tu, h45.x, h23.y);
+        hi = fma(Tu, hi, h23.x);
+        hi = fma(Tu, hi, h01.y);
+        hi = fma(Tu, hi, h6w.x);
+        hi = fma(h45.y, c.rT[0], hi);
+        hi = fma(h01.x, oml, hi);
+        const double g2 = Tu <= l6t.y ? lo : hi;
+        const double z = y * h6w.y;
+        invW += z;
+        *reinterpret_cast<double2 *>(sL + (size_t)k * 2048) = make_double2(z, exp2c(lc02 - g2));
+        *reinterpret_cast<double *>(om + (size_t)k * 1024) = 0.0;
+    }
+    *reinterpret_cast<double2 *>(sL + (size_t)Ns * 2048) = make_double2(1.0, 1.0);
+    *reinterpret_cast<double *>(om + (size_t)Ns * 1024) = 0.0;
+    const double rho = pi / (CRF_R_GAS * Tu * invW);
+    for (int k = 0; k < Ns; ++k) *reinterpret_cast<double *>(sL + (size_t)k * 2048) *= rho;  // C_k
+    __syncthreads();  // the tables have landed (the state and omega columns are private to the thread)
+
+    for (int ci = 0; ci < rs.n_chunks; ++ci) {
+        const int4 ch = __ldg(rs.chunk + ci);
+        const char *blk = sTab + ch.z;
+        const int count = ch.y, o_troe = 48 * count + 32;  // one slot row (W = 1, maxown = 4) follows the records
+        switch (ch.x) {
+        case 0: thread_chunk<0, false>(blk, count, o_troe, sL, om, c); break;
+        case 1: thread_chunk<1, false>(blk, count, o_troe, sL, om, c); break;
+        case 2: thread_chunk<2, false>(blk, count, o_troe, sL, om, c); break;
+        default: thread_chunk<0, true>(blk, count, o_troe, sL, om, c); break;
+        }
+    }
+
+    // ---- store omega; a9: qdot = -sum_k h_k omega_k
+    double qd = 0.0;
+    for (int k = 0; k < Ns; ++k) {
+        const double2 *h = reinterpret_cast<const double2 *>(rs.hco + 16 * (size_t)k);
+        const double2 l01 = __ldg(h), l23 = __ldg(h + 1), l45 = __ldg(h + 2), l6t = __ldg(h + 3);
+        const double2 h01 = __ldg(h + 4), h23 = __ldg(h + 5), h45 = __ldg(h + 6);
+        double lo = fma(Tu, l45.x, l23.y);
+        lo = fma(Tu, lo, l23.x);
+        lo = fma(Tu, lo, l01.y);
+        lo = fma(Tu, lo, l01.x);
+        lo = fma(l45.y, c.rT[0], lo);
+        double hi = fma(Tu, h45.x, h23.y);
+        hi = fma(Tu, hi, h23.x);
+        hi = fma(Tu, hi, h01.y);
+        hi = fma(Tu, hi, h01.x);
+        hi = fma(h45.y, c.rT[0], hi);
+        const double w = *reinterpret_cast<const double *>(om + (size_t)k * 1024);
+        qd = fma(-(Tu <= l6t.y ? lo : hi), w, qd);
+        if (i < n) omega[(int64_t)k * n + i] = w;
+    }
+    if (i < n) qdot[i] = qd * (CRF_R_GAS * Tu);
+}
+
+cudaError_t launch_thread(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
+                          double *qdot, cudaStream_t st)
+{
+    const size_t smem = (size_t)(m.Ns + 1) * (2048 + 1024) + (size_t)m.rs.stage_bytes;
+    cudaError_t e = cudaFuncSetAttribute(rates_thread_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    rates_thread_kernel<<<(unsigned)((n + RT_B - 1) / RT_B), RT_B, smem, st>>>(m, T, p, Y, n, omega, qdot);
+    crf_count_launch();
+    return cudaGetLastError();
+}
+
 }  // namespace
 
 cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
@@ -460,6 +602,7 @@ cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double 
 {
     const int key = m.rs.W * 10 + m.rs.PPL;
     switch (key) {
+    case 14: return launch_thread(m, T, p, Y, n, omega, qdot, st);
     case 41: return launch_wp<4, 1>(m, T, p, Y, n, omega, qdot, st);
     case 42: return launch_wp<4, 2>(m, T, p, Y, n, omega, qdot, st);
     case 81: return launch_wp<8, 1>(m, T, p, Y, n, omega, qdot, st);

@@ -211,11 +211,13 @@ PLAN_OVERRIDES = [
     {"CRF_RATES_W": "8", "CRF_RATES_PPL": "1"},
     {"CRF_RATES_W": "4", "CRF_RATES_PPL": "2", "CRF_RATES_RC": "32"},   # many small chunks
     {"CRF_RATES_SMEM": "0"},                           # the staged fallback kernel
+    {"CRF_RATES_THREAD": "1"},                         # one thread per point (admitted for Ns <= 24: C3 here)
+    {"CRF_TRANSPORT_SMALL": "0"},                      # generic transport kernel (only differs for Ns <= 16)
 ]
 
 
 @pytest.mark.parametrize("env", PLAN_OVERRIDES, ids=lambda e: ",".join(f"{k[4:]}={v}" for k, v in e.items()))
-@pytest.mark.parametrize("name", ["C3", "C4", "C5"])
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
 def test_plan_overrides(binding, oracle_mod, monkeypatch, name, env):
     """The kernel plans are chosen in crf_mech_create; the CRF_* tuning overrides select the other template
     instances (warps per point group, points per lane, chunk size, fallback kernel): each must meet the same
