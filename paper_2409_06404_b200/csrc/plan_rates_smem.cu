@@ -216,6 +216,7 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
             blocks.push_back(chunk_block(B, ch, PPL, W, maxown));
             stage_bytes = std::max(stage_bytes, (blocks.back().size() + 15) & ~size_t(15));
         }
+        stage_bytes = std::max(stage_bytes, (size_t)128 * Ns);  // the buffers also carry the NASA sets (prologue, epilogue)
         Rc = cand;
         if (state(PPL) + (size_t)cand * 256 * PPL + 2 * stage_bytes <= budget(W)) break;
         if (cand == step) return o;  // does not fit at all

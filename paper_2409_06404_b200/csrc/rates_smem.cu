@@ -244,6 +244,8 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     double *sred = reinterpret_cast<double *>(sQ);            // [W][PPL][32], valid outside the chunk loop
 
     stage_async(sStage, rs.stage + __ldg(&rs.chunk[0].z), rs.stage_bytes, threadIdx.x, 32 * W);
+    // the second stage buffer is free until chunk 1 is prefetched: it carries the g/(RT) sets for the prologue
+    stage_async(sStage + rs.stage_bytes, reinterpret_cast<const unsigned char *>(rs.gco), 128 * Ns, threadIdx.x, 32 * W);
 
     const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * PPL;
     const bool vec = (n & 1) == 0;
@@ -259,6 +261,9 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         c.Csum[u] = pi[u] * c.rT[u] * (1.0 / CRF_R_GAS);
     }
 
+    stage_wait();
+    __syncthreads();
+    const double2 *sG = reinterpret_cast<const double2 *>(sStage + rs.stage_bytes);
     // ---- a1, a2: Z_k = Y_k/W_k and d_k = 2^(log2(p_ref/RT) - log2e g_k/RT); warp w takes species w, w+W, ...
     double invW[PPL];
 #pragma unroll
@@ -276,9 +281,9 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         for (int j = 0; j < 4; ++j) {
             const int k = warp + W * (s0 + j);
             if (k >= Ns) continue;
-            const double2 *g = reinterpret_cast<const double2 *>(rs.gco + 16 * (size_t)k);
-            const double2 l01 = __ldg(g), l23 = __ldg(g + 1), l45 = __ldg(g + 2), l6t = __ldg(g + 3);
-            const double2 h01 = __ldg(g + 4), h23 = __ldg(g + 5), h45 = __ldg(g + 6), h6w = __ldg(g + 7);
+            const double2 *g = sG + 8 * k;
+            const double2 l01 = g[0], l23 = g[1], l45 = g[2], l6t = g[3];
+            const double2 h01 = g[4], h23 = g[5], h45 = g[6], h6w = g[7];
 #pragma unroll
             for (int u = 0; u < PPL; ++u) {
                 const double Tu = c.T[u], oml = 1.0 - c.L[u];
@@ -337,6 +342,9 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         if (ci + 1 < nch)
             stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, rs.stage + __ldg(&rs.chunk[ci + 1].z),
                         rs.stage_bytes, threadIdx.x, 32 * W);
+        else  // behind the last chunk: the h/(RT) sets for the epilogue
+            stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, reinterpret_cast<const unsigned char *>(rs.hco),
+                        128 * Ns, threadIdx.x, 32 * W);
         const int count = ch.y;
         constexpr int SLOT_ROW = 16 + 4 * MAXOWN;
         const int o_slot = 48 * count, o_troe = o_slot + SLOT_ROW * W;
@@ -390,9 +398,9 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     for (int s = 0; s < MAXOWN; ++s) {
         const int k = warp + W * s;
         if (k < Ns) {
-            const double2 *h = reinterpret_cast<const double2 *>(rs.hco + 16 * (size_t)k);
-            const double2 l01 = __ldg(h), l23 = __ldg(h + 1), l45 = __ldg(h + 2), l6t = __ldg(h + 3);
-            const double2 h01 = __ldg(h + 4), h23 = __ldg(h + 5), h45 = __ldg(h + 6);
+            const double2 *h = reinterpret_cast<const double2 *>(sStage + (size_t)(nch & 1) * rs.stage_bytes) + 8 * k;
+            const double2 l01 = h[0], l23 = h[1], l45 = h[2], l6t = h[3];
+            const double2 h01 = h[4], h23 = h[5], h45 = h[6];
 #pragma unroll
             for (int u = 0; u < PPL; ++u) {
                 const double Tu = c.T[u];
