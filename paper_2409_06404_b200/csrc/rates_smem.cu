@@ -146,7 +146,12 @@ __device__ __forceinline__ void reaction_q(const char *blk, const char *rec, con
             const double2 a2 = lds2(s + x0), b2 = lds2(s + x1);
             Pf *= a2.x, Pr *= b2.x, num *= a2.y, den *= b2.y;
         }
-        const double net = fma(-(num * rcp_fast(den)), Pr, Pf);  // prod C_reactants - prod C_products / K_c
+        // 1/K_c = num/den with the MUFU seed and ONE Newton step (relative error 2^-40: the tolerance of omega is
+        // 1e-10 of the gross rate); net = prod C_reactants - prod C_products / K_c
+        double ry;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(ry) : "d"(den));
+        const double t0 = num * ry;
+        const double net = fma(-fma(t0, fma(-den, ry, 1.0), t0), Pr, Pf);
         if (KIND == 0) q[u] = exp2c(yinf) * net;
         if (KIND == 1) q[u] = exp2c(yinf) * M[u] * net;
         if (KIND == 2) {
