@@ -93,6 +93,8 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
     if (W != 1 && W != 2 && W != 4 && W != 8) {
         W = 1;
         while (W < 8 && W < per_round) W *= 2;
+        if (nb <= 3) W = 1;  // a round of nb = 3 is one full tile and one diagonal tile: two warps would idle 28 %
+                             // (C3: W = 1 3.0 ms, W = 2 4.1 ms); the state is small, so the SM still holds 16 blocks
     }
     int PPL = env_int("CRF_TRANSPORT_PPL", 1);
     if (PPL != 1 && PPL != 2) PPL = 1;
