@@ -229,3 +229,28 @@ def test_plan_overrides(binding, oracle_mod, monkeypatch, name, env):
     n = SMALL_N[name] + 2
     st = wl.make_state(name, n=n, total=n)
     parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), f"{name} {env} n={n}")
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_extreme_states(binding, oracle_mod, name):
+    """The corners of the range the kernels are specified for (crf_mech_create admits the product form of
+    K_c for 250 K <= T <= 5000 K): very cold and very hot points, low and high pressure, mass fractions
+    with exact zeros, a dominant species and traces down to 1e-30, next to ordinary points in the same warp."""
+    desc, gm, om = _mech_pair(binding, oracle_mod, name)
+    Ns = gm.Ns
+    rng = np.random.default_rng(11)
+    Ts = np.array([255.0, 300.0, 650.0, 1000.0, 1800.0, 3000.0, 4200.0, 4950.0])
+    ps = np.array([1.0e3, 1.0e5, 1.0e7])
+    T, p = (a.ravel() for a in np.meshgrid(Ts, ps, indexing="ij"))
+    T, p = np.tile(T, 5), np.tile(p, 5)  # 120 points: several warps, mixed extremes in each
+    n = T.size
+    Y = rng.dirichlet(np.full(Ns, 0.3), size=n).T
+    Y[rng.random(Y.shape) < 0.25] = 0.0
+    Y[rng.random(Y.shape) < 0.10] = 1e-30
+    Y[rng.integers(0, Ns, n // 3), np.arange(0, n, 3)[: n // 3]] += 5.0  # one dominant species at every third point
+    Y /= Y.sum(axis=0)
+    st = dict(T=T, p=p, Y=np.ascontiguousarray(Y))
+    gpu, ref = parity.run_gpu(gm, st), parity.run_oracle(om, st)
+    for key in ("cp", "h", "mu", "lam", "rhoD", "omega", "qdot"):
+        assert np.all(np.isfinite(gpu[key])) and np.all(np.isfinite(ref[key])), key
+    parity.assert_parity(gpu, ref, f"{name} extreme states")
