@@ -174,9 +174,9 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
     // Small mechanisms: one THREAD per point (rates_thread_kernel in rates_smem.cu), 128 points per block, the (C, d)
     // state and omega as per-thread columns in shared memory (row stride 128 x 16 bytes = the layout of "4 points
     // per lane"), all chunk blocks resident at once.  Marked W = 1, PPL = 4; stage_bytes = all blocks.
-    // Opt-in (CRF_RATES_THREAD=1): measured no faster than the warp-group kernel (C2 3.4 vs 3.4 ms, C3 3.2 vs 2.6 ms):
-    // fewer instructions per point, but the per-thread dependent shared-memory chains are not hidden.
-    if (Ns <= 24 && env_int("CRF_RATES_THREAD", 0) != 0 && env_int("CRF_RATES_W", 0) == 0) {
+    // Default for Ns <= 12 (C2: 2.96 ms against 3.40 ms for the warp-group kernel); opt-in up to Ns = 24 with
+    // CRF_RATES_THREAD=1 (C3: 3.9 against 2.4 ms: the per-thread shared-memory chains are not hidden at 12 warps per SM).
+    if (Ns <= 24 && env_int("CRF_RATES_THREAD", Ns <= 12 ? 1 : 0) != 0 && env_int("CRF_RATES_W", 0) == 0) {
         chunks = make_chunks(B, Nr);
         for (const Chunk &ch : chunks) {
             blocks.push_back(chunk_block(B, ch, 4, 1, 4));

@@ -476,6 +476,14 @@ constexpr int RT_B = 128;
 __device__ __forceinline__ void scatter_q(char *om, const char *rec, double q, bool generic)
 {
     const uint4 S = ldsu4(rec + 32);  // state row offsets (stride 2048) -> omega rows (stride 1024)
+    if (!generic && S.x != S.y && S.z != S.w && S.x != S.z && S.x != S.w && S.y != S.z && S.y != S.w) {
+        // four distinct rows (a warp-uniform test): the four loads go out together, then the four stores
+        double *r0 = reinterpret_cast<double *>(om + (S.x >> 1)), *r1 = reinterpret_cast<double *>(om + (S.y >> 1));
+        double *r2 = reinterpret_cast<double *>(om + (S.z >> 1)), *r3 = reinterpret_cast<double *>(om + (S.w >> 1));
+        const double v0 = *r0, v1 = *r1, v2 = *r2, v3 = *r3;
+        *r0 = v0 - q, *r1 = v1 - q, *r2 = v2 + q, *r3 = v3 + q;
+        return;
+    }
     *reinterpret_cast<double *>(om + (S.x >> 1)) -= q;
     *reinterpret_cast<double *>(om + (S.y >> 1)) -= q;
     *reinterpret_cast<double *>(om + (S.z >> 1)) += q;
@@ -517,8 +525,14 @@ __global__ void __launch_bounds__(RT_B) rates_thread_kernel(DevTables m, const d
     char *sCD = reinterpret_cast<char *>(sm2);        // [Ns + 1][128] (C_k, d_k); row Ns = (1, 1)
     char *sOm = sCD + (size_t)(Ns + 1) * 2048;        // [Ns + 1][128] omega_k; row Ns collects the empty slots
     char *sTab = sOm + (size_t)(Ns + 1) * 1024;       // the chunk blocks
+    char *sGH = sTab + rs.stage_bytes;                // g/(RT) sets [Ns][128 B], then h/(RT) sets [Ns][128 B]
     for (int o = tid * 16; o < rs.stage_bytes; o += RT_B * 16)
         *reinterpret_cast<uint4 *>(sTab + o) = __ldg(reinterpret_cast<const uint4 *>(rs.stage + o));
+    for (int o = tid * 16; o < 128 * Ns; o += RT_B * 16) {
+        *reinterpret_cast<uint4 *>(sGH + o) = __ldg(reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(rs.gco) + o));
+        *reinterpret_cast<uint4 *>(sGH + 128 * Ns + o) =
+            __ldg(reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(rs.hco) + o));
+    }
     char *sL = sCD + tid * 16, *om = sOm + tid * 8;
 
     const int64_t i = (int64_t)blockIdx.x * RT_B + tid;
@@ -532,12 +546,20 @@ __global__ void __launch_bounds__(RT_B) rates_thread_kernel(DevTables m, const d
     c.Csum[0] = pi * c.rT[0] * (1.0 / CRF_R_GAS);
     const double oml = 1.0 - c.L[0];
 
+    __syncthreads();  // the tables have landed (the state and omega columns are private to the thread)
     double invW = 0.0;
-    for (int k = 0; k < Ns; ++k) {
-        const double2 *g = reinterpret_cast<const double2 *>(rs.gco + 16 * (size_t)k);
-        const double2 l01 = __ldg(g), l23 = __ldg(g + 1), l45 = __ldg(g + 2), l6t = __ldg(g + 3);
-        const double2 h01 = __ldg(g + 4), h23 = __ldg(g + 5), h45 = __ldg(g + 6), h6w = __ldg(g + 7);
-        const double y = Y[(int64_t)k * n + ic];
+    for (int k0 = 0; k0 < Ns; k0 += 4) {
+      double y4[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) y4[j] = Y[(int64_t)min(k0 + j, Ns - 1) * n + ic];  // four row loads in flight
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int k = k0 + j;
+        if (k >= Ns) break;
+        const double2 *g = reinterpret_cast<const double2 *>(sGH) + 8 * k;
+        const double2 l01 = g[0], l23 = g[1], l45 = g[2], l6t = g[3];
+        const double2 h01 = g[4], h23 = g[5], h45 = g[6], h6w = g[7];
+        const double y = y4[j];
         double lo = fma(Tu, l45.x, l23.y);
         lo = fma(Tu, lo, l23.x);
         lo = fma(Tu, lo, l01.y);
@@ -555,12 +577,12 @@ __global__ void __launch_bounds__(RT_B) rates_thread_kernel(DevTables m, const d
         invW += z;
         *reinterpret_cast<double2 *>(sL + (size_t)k * 2048) = make_double2(z, exp2c(lc02 - g2));
         *reinterpret_cast<double *>(om + (size_t)k * 1024) = 0.0;
+      }
     }
     *reinterpret_cast<double2 *>(sL + (size_t)Ns * 2048) = make_double2(1.0, 1.0);
     *reinterpret_cast<double *>(om + (size_t)Ns * 1024) = 0.0;
     const double rho = pi / (CRF_R_GAS * Tu * invW);
     for (int k = 0; k < Ns; ++k) *reinterpret_cast<double *>(sL + (size_t)k * 2048) *= rho;  // C_k
-    __syncthreads();  // the tables have landed (the state and omega columns are private to the thread)
 
     for (int ci = 0; ci < rs.n_chunks; ++ci) {
         const int4 ch = __ldg(rs.chunk + ci);
@@ -577,9 +599,9 @@ __global__ void __launch_bounds__(RT_B) rates_thread_kernel(DevTables m, const d
     // ---- store omega; a9: qdot = -sum_k h_k omega_k
     double qd = 0.0;
     for (int k = 0; k < Ns; ++k) {
-        const double2 *h = reinterpret_cast<const double2 *>(rs.hco + 16 * (size_t)k);
-        const double2 l01 = __ldg(h), l23 = __ldg(h + 1), l45 = __ldg(h + 2), l6t = __ldg(h + 3);
-        const double2 h01 = __ldg(h + 4), h23 = __ldg(h + 5), h45 = __ldg(h + 6);
+        const double2 *h = reinterpret_cast<const double2 *>(sGH + 128 * Ns) + 8 * k;
+        const double2 l01 = h[0], l23 = h[1], l45 = h[2], l6t = h[3];
+        const double2 h01 = h[4], h23 = h[5], h45 = h[6];
         double lo = fma(Tu, l45.x, l23.y);
         lo = fma(Tu, lo, l23.x);
         lo = fma(Tu, lo, l01.y);
@@ -600,7 +622,7 @@ __global__ void __launch_bounds__(RT_B) rates_thread_kernel(DevTables m, const d
 cudaError_t launch_thread(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
                           double *qdot, cudaStream_t st)
 {
-    const size_t smem = (size_t)(m.Ns + 1) * (2048 + 1024) + (size_t)m.rs.stage_bytes;
+    const size_t smem = (size_t)(m.Ns + 1) * (2048 + 1024) + (size_t)m.rs.stage_bytes + 256 * (size_t)m.Ns;
     cudaError_t e = cudaFuncSetAttribute(rates_thread_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     rates_thread_kernel<<<(unsigned)((n + RT_B - 1) / RT_B), RT_B, smem, st>>>(m, T, p, Y, n, omega, qdot);

@@ -211,7 +211,8 @@ PLAN_OVERRIDES = [
     {"CRF_RATES_W": "8", "CRF_RATES_PPL": "1"},
     {"CRF_RATES_W": "4", "CRF_RATES_PPL": "2", "CRF_RATES_RC": "32"},   # many small chunks
     {"CRF_RATES_SMEM": "0"},                           # the staged fallback kernel
-    {"CRF_RATES_THREAD": "1"},                         # one thread per point (admitted for Ns <= 24: C3 here)
+    {"CRF_RATES_THREAD": "1"},                         # one thread per point (default for Ns <= 12; C3 here)
+    {"CRF_RATES_THREAD": "0"},                         # ... and the warp-group kernel where that is the default (C2)
     {"CRF_TRANSPORT_SMALL": "0"},                      # generic transport kernel (only differs for Ns <= 16)
 ]
 
