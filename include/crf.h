@@ -147,6 +147,12 @@ int crf_fp64_probe(int iters, double *inst_per_s);
 /* How many kernel launches this library has issued in this process (for bench.py). */
 int64_t crf_launch_count(void);
 
+/* Host-only diagnostic (no device needed): the tile schedule crf_mech_create lays out for crf_mix_transport on a
+ * mechanism whose species fill nb blocks of 8, dealt to W warps.  Writes up to `cap` tiles as
+ * int32 quadruples {round, kind (1 off-diagonal, 2 diagonal), jb, kb} to out and returns the number of tiles
+ * of the schedule (which may exceed cap), or CRF_EINVAL. */
+int crf_transport_schedule(int nb, int W, int32_t *out, int cap);
+
 const char *crf_last_error(void);
 
 #ifdef __cplusplus

@@ -18,7 +18,8 @@ _lib = None
 
 EXPORTS = ("crf_mech_create", "crf_mech_destroy", "crf_mech_set_stream", "crf_mech_num_species",
            "crf_mech_num_reactions", "crf_thermo", "crf_thermo_species", "crf_production_rates",
-           "crf_mix_transport", "crf_step_host", "crf_fp64_probe", "crf_launch_count", "crf_last_error")
+           "crf_mix_transport", "crf_step_host", "crf_fp64_probe", "crf_launch_count", "crf_transport_schedule",
+           "crf_last_error")
 
 
 class CrfError(RuntimeError):

@@ -177,3 +177,20 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
     o.rounds = b.add(rdesc), o.pair_coef = b.add(coef), o.wilke_cP = b.add(cP), o.sp = b.add(sp), o.Ddiag = b.add(dd);
     return o;
 }
+
+extern "C" int crf_transport_schedule(int nb, int W, int32_t *out, int cap)
+{
+    if (nb < 1 || nb > 255 || W < 1 || W > 8 || (cap > 0 && !out)) return CRF_EINVAL;
+    int count = 0, rd = 0;
+    for (auto &round : schedule_rounds(nb, W)) {
+        for (const Tile &tl : round) {
+            if (count < cap) {
+                int32_t *o = out + 4 * (size_t)count;
+                o[0] = rd, o[1] = tl.kind, o[2] = tl.jb, o[3] = tl.kb;
+            }
+            ++count;
+        }
+        ++rd;
+    }
+    return count;
+}

@@ -132,3 +132,30 @@ def test_generator_matches_config_recipes():
         st = wl.make_state(name, n=1024, total=1024)
         assert st["Y"].shape == (cfg["Ns"], 1024) and np.allclose(st["Y"].sum(axis=0), 1.0, atol=1e-14)
         assert st["Y"].min() > 0 and st["T"].min() > 250 and st["T"].max() < 2700
+
+
+@pytest.mark.parametrize("nb", list(range(1, 18)) + [31, 32])
+@pytest.mark.parametrize("W", [1, 2, 4, 8])
+def test_transport_tile_schedule(lib_path, nb, W):
+    """Host logic of the tiled transport kernel (no GPU): the round-robin schedule must visit every unordered pair
+    of species blocks and every diagonal block exactly once, a round must hold at most W tiles, and the tiles of a
+    round must touch pairwise disjoint blocks (that is what lets the warps update S without atomics)."""
+    L = binding.lib()
+    L.crf_transport_schedule.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int]
+    total = nb * (nb - 1) // 2 + nb
+    buf = (C.c_int32 * (4 * total))()
+    assert L.crf_transport_schedule(nb, W, buf, total) == total
+    tiles = np.frombuffer(buf, dtype=np.int32).reshape(total, 4)
+    seen = set()
+    for rd in np.unique(tiles[:, 0]):
+        t = tiles[tiles[:, 0] == rd]
+        assert len(t) <= W
+        blocks = []
+        for _, kind, jb, kb in t:
+            assert 0 <= jb <= kb < nb and kind == (2 if jb == kb else 1)
+            blocks += [jb] if jb == kb else [jb, kb]
+            assert (jb, kb) not in seen
+            seen.add((jb, kb))
+        assert len(blocks) == len(set(blocks)), f"round {rd} touches a block twice"
+    assert len(seen) == total
+    assert L.crf_transport_schedule(0, W, None, 0) == -1 and L.crf_transport_schedule(nb, 3 * W + 9, None, 0) == -1
