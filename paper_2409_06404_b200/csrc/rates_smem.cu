@@ -74,37 +74,6 @@ __device__ __forceinline__ double log2_fast(double x)
     return fma(s * (2.0 * crf::kLog2e), p, (double)e);
 }
 
-// shared memory through 32-bit shared-window addresses (no generic-pointer arithmetic in the hot loops)
-__device__ __forceinline__ double2 lds_d2(unsigned a)
-{
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ double lds_d(unsigned a)
-{
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ uint4 lds_u4(unsigned a)
-{
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ unsigned lds_u(unsigned a)
-{
-    unsigned v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ void sts_d(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
-__device__ __forceinline__ void sts_d2(unsigned a, double x, double y)
-{
-    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
-}
-
 template <int PPL>
 struct Ctx {
     double T[PPL], L[PPL], rT[PPL];  // T, ln T, 1/T
