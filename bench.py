@@ -165,8 +165,16 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def host_cores_for_the_oracle():
+    """torchrun exports OMP_NUM_THREADS=1 to every rank.  The CPU baseline is defined on the box's host cores and only
+    rank 0 runs it, so that setting is dropped before any OpenMP runtime is loaded (torch's or the oracle's)."""
+    if "TORCHELASTIC_RUN_ID" in os.environ and os.environ.get("OMP_NUM_THREADS") == "1":
+        os.environ.pop("OMP_NUM_THREADS")
+
+
 def main():
     args = parse()
+    host_cores_for_the_oracle()
     if args.impl == "reference":
         return reference_arm(args)
 
