@@ -223,6 +223,7 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
     }
     o.W = W, o.PPL = PPL, o.maxown = maxown, o.Rc = Rc;
     }
+    if (chunks.size() > 64) return RatesSmemPlanOffsets();  // the kernel keeps at most 64 chunk descriptors
     o.n_chunks = (int)chunks.size(), o.stage_bytes = (int)stage_bytes;
 
     std::vector<int4> cdesc;

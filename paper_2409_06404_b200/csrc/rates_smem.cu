@@ -217,6 +217,10 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     char *sQl = sQ + lane * 8;
     double *sred = reinterpret_cast<double *>(sQ);            // [W][PPL][32], valid outside the chunk loop
 
+    // chunk descriptors: read once, before the loop needs them (a global load at the top of every chunk would put
+    // an L2 round trip on every warp's critical path)
+    __shared__ int4 sChunk[64];
+    for (int ci = threadIdx.x; ci < rs.n_chunks && ci < 64; ci += 32 * W) sChunk[ci] = __ldg(rs.chunk + ci);
     stage_async(sStage, rs.stage + __ldg(&rs.chunk[0].z), rs.stage_bytes, threadIdx.x, 32 * W);
     // the second stage buffer is free until chunk 1 is prefetched: it carries the g/(RT) sets for the prologue
     stage_async(sStage + rs.stage_bytes, reinterpret_cast<const unsigned char *>(rs.gco), 128 * Ns, threadIdx.x, 32 * W);
@@ -311,10 +315,10 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
 
     const int nch = rs.n_chunks;
     for (int ci = 0; ci < nch; ++ci) {
-        const int4 ch = __ldg(rs.chunk + ci);
+        const int4 ch = sChunk[ci];
         const char *blk = sStage + (size_t)(ci & 1) * rs.stage_bytes;
         if (ci + 1 < nch)
-            stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, rs.stage + __ldg(&rs.chunk[ci + 1].z),
+            stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, rs.stage + sChunk[ci + 1].z,
                         rs.stage_bytes, threadIdx.x, 32 * W);
         else  // behind the last chunk: the h/(RT) sets for the epilogue
             stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, reinterpret_cast<const unsigned char *>(rs.hco),
