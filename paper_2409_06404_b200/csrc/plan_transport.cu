@@ -125,8 +125,9 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
         stage_bytes = std::max(stage_bytes, 8 * (coef.size() - start));
     };
     // Wilke stage blocks: pass p covers the row blocks p W .. p W + W - 1 (one per warp), a panel covers up to
-    // kPanel column blocks; payload [W][8 rows][8 nJ columns] of c_kj (0 in padded rows/columns)
-    const int kPanel = 3, npass = (nb + W - 1) / W;
+    // kPanel column blocks (as many as keep the block within 20 KB: fewer, larger stage steps measured faster, C5 panel
+    // 3 -> 5 29.2 -> 28.8 ms, C4 15.5 -> 15.0 ms; CRF_TRANSPORT_PANEL overrides); payload [W][8 rows][8 nJ columns] of c_kj (0 in padded rows/columns)
+    const int kPanel = std::max(1, env_int("CRF_TRANSPORT_PANEL", std::min({nb, 5, 20480 / (W * 512)}))), npass = (nb + W - 1) / W;
     for (int ps = 0; ps < npass; ++ps)
         for (int J0 = 0; J0 < nb; J0 += kPanel) {
             const int nJ = std::min(kPanel, nb - J0);
