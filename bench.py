@@ -35,7 +35,7 @@ UNIT = "points/s"
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
@@ -76,6 +76,20 @@ def run_oracle_sample(name, m_points):
     return m_points / dt, crf_oracle.max_threads(), dt
 
 
+def run_oracle_one_core(name, m_points):
+    """The same oracle sample on ONE host core ('all cores ... and additionally 1 core'): a child
+    process with OMP_NUM_THREADS=1, so that the OpenMP team of this process is left alone."""
+    code = ("import sys, json; sys.path.insert(0, %r); import bench; "
+            "v, c, dt = bench.run_oracle_sample(%r, %d); print(json.dumps([v, c, dt]))" % (ROOT, name, m_points))
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+        v, c, dt = json.loads(out.stdout.strip().splitlines()[-1])
+        return v, int(c), dt
+    except Exception:  # noqa: BLE001  (a reported baseline: never fail the bench line over it)
+        return None, 1, None
+
+
 def reference_arm(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -104,17 +118,22 @@ def reference_arm(args):
     return 0
 
 
-def ncu_traffic(workload, kernel):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on `workload`, from the committed
-    ncu --set full summary (profiles/r01_dram_traffic.csv: a measurement made under the profiler, not by this run)."""
-    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+def ncu_counters(workload, kernel):
+    """Counters of one launch of `kernel` on `workload` from the committed ncu --set full summary
+    (profiles/r02_ncu_counters.csv: measured under the profiler on the build named there, not by this run):
+    dict(traffic = dram__bytes_read.sum + dram__bytes_write.sum, fp64_inst = thread-level FP64 pipe instructions
+    executed, inst = thread-level instructions executed) or None."""
+    path = os.path.join(ROOT, "profiles", "r02_ncu_counters.csv")
     try:
         with open(path) as f:
-            for row in f.read().splitlines()[1:]:
-                c = row.split(",")
-                if len(c) >= 4 and c[0] == workload and c[1] == kernel:
-                    return float(c[2]) + float(c[3])
-    except OSError:
+            rows = [r.split(",") for r in f.read().splitlines() if r and not r.startswith("#")]
+        hdr = rows[0]
+        for c in rows[1:]:
+            d = dict(zip(hdr, c))
+            if d.get("workload") == workload and d.get("call") == kernel:
+                return dict(traffic=float(d["dram_read_bytes"]) + float(d["dram_write_bytes"]),
+                            fp64_inst=float(d["fp64_thread_inst"]), inst=float(d["thread_inst"]), build=d.get("build"))
+    except (OSError, KeyError, ValueError, IndexError):
         pass
     return None
 
@@ -258,6 +277,7 @@ def main():
     if flush is not None:  # the flush is not part of the step: time the three calls only
         total_ms = float(per_kernel.sum())
     kern_ms = per_kernel.mean(axis=0)
+    kern_med, kern_best = np.median(per_kernel, axis=0), per_kernel.min(axis=0)
 
     # ---- end to end through crf_step_host: pinned host in, pinned host out
     e2e = None
@@ -306,11 +326,21 @@ def main():
         w, ms = work[nm], float(kern_ms[i])
         t_alu = w["F"] * n / (rooflines.FP64_PEAK_TFLOPS * 1e12)
         t_hbm = w["B"] * n / (peaks["hbm_gbs"] * 1e9)
-        kernels[nm] = {"ms": ms, "share": ms / float(kern_ms.sum()), "points_per_s": n / (ms * 1e-3),
+        t_inst = w["I"] * n / rooflines.FP64_PEAK_INST
+        kernels[nm] = {"ms": ms, "ms_median": float(kern_med[i]), "ms_best": float(kern_best[i]),
+                       "share": ms / float(kern_ms.sum()), "points_per_s": n / (ms * 1e-3),
                        "bound": "alu" if t_alu >= t_hbm else "hbm", "tflops": w["F"] * n / (ms * 1e-3) / 1e12,
-                       "gbs": w["B"] * n / (ms * 1e-3) / 1e9, "frac_of_roofline": max(t_alu, t_hbm) / (ms * 1e-3)}
+                       "gbs": w["B"] * n / (ms * 1e-3) / 1e9, "frac_of_roofline": max(t_alu, t_hbm) / (ms * 1e-3),
+                       # the same fraction with the algorithmic work counted in FP64 instructions instead of flops
+                       "frac_instr_basis": max(t_inst, t_hbm) / (ms * 1e-3)}
+        ctr = ncu_counters(name, nm)
+        if ctr:  # what the shipped kernel executes (ncu, committed): FP64 pipe issue rate against the pipe's peak
+            kernels[nm]["frac_executed_fp64"] = ctr["fp64_inst"] / rooflines.FP64_PEAK_INST / (ms * 1e-3)
+            kernels[nm]["fp64_share_of_executed_inst"] = ctr["fp64_inst"] / ctr["inst"]
+            kernels[nm]["dram_traffic_over_algorithmic"] = ctr["traffic"] / (w["B"] * n) if args.points == 0 else None
     dom = max(names, key=lambda k: kernels[k]["ms"])
-    traffic = ncu_traffic(name, dom)
+    ctr = ncu_counters(name, dom)
+    traffic = ctr["traffic"] if ctr and args.points == 0 else None
     kd = kernels[dom]
     if kd["bound"] == "alu":
         roof = {"bound": "alu", "kernel": dom, "achieved": kd["tflops"], "peak": rooflines.FP64_PEAK_TFLOPS,
@@ -328,8 +358,12 @@ def main():
     if not args.no_cpu:
         m = min(n, args.cpu_points or CPU_SAMPLE[name])
         v, cores, dt = run_oracle_sample(name, m)
+        m1 = max(512, m // max(cores, 1))
+        v1, _, dt1 = run_oracle_one_core(name, m1)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"first {m} points of {name}, thermo+rates+transport, gcc -O2 OpenMP, {dt:.1f} s"}
+               "sample": f"first {m} points of {name}, thermo+rates+transport, gcc -O2 OpenMP, {dt:.1f} s",
+               "value_1core": v1, "sample_1core": f"first {m1} points of {name}, OMP_NUM_THREADS=1"
+                                                  + (f", {dt1:.1f} s" if dt1 else " (failed)")}
 
     line = {"metric": METRIC, "value": world * n * K / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",

@@ -23,8 +23,16 @@
  *  - Calls are asynchronous on the mechanism's stream (crf_mech_set_stream, default: the
  *    legacy default stream) and do not synchronise.
  *  - Return 0 (CRF_OK) or a negative code; crf_last_error() gives the text of the last
- *    failure on the calling thread.  Non-finite or unphysical inputs (T <= 0) are not
- *    checked; outputs are then unspecified.  No C++ exception crosses this boundary.
+ *    failure on the calling thread.  No C++ exception crosses this boundary.
+ *  - Validated input range: 250 K <= T <= 5000 K, p > 0, finite Y.  crf_mech_create admits the
+ *    fast form of the equilibrium constant (a product of per-species factors instead of a second
+ *    exponential per reaction) only if every factor stays inside the double range over that
+ *    temperature window; otherwise it selects the log-space kernel by itself.  Outside the
+ *    window (and for non-finite inputs or T <= 0, which are not checked) outputs are
+ *    unspecified: rate constants that underflow are flushed towards zero, nothing traps.
+ *  - Kernel plans (warps per point group, chunk sizes, which kernel variant) are chosen by
+ *    crf_mech_create from the mechanism's size; no environment variable is read.  Explicit
+ *    plan options and the diagnostics live in crf_diag.h.
  */
 #ifndef CRF_H
 #define CRF_H
@@ -42,6 +50,7 @@ extern "C" {
 
 #define CRF_TABLES_VERSION 1
 #define CRF_MAX_SLOTS 3 /* reactant (and product) slots per reaction */
+#define CRF_MAX_SPECIES 220 /* largest Ns crf_mech_create accepts (per-point state in shared memory) */
 
 /* Host-side species-major SoA mechanism tables, produced by the packer
  * (paper_2409_06404_b200/packer.py) from a mechanism description.  All pointers are HOST
@@ -80,7 +89,9 @@ typedef struct crf_tables {
     const double *eff_val;  /* [eff_ptr[N3+Nt]] */
 
     /* Troe falloff, one entry per falloff reaction: low-pressure limit k0 and
-     * F_cent = (1-alpha) exp(-T/T3) + alpha exp(-T/T1) + exp(-T2/T) */
+     * F_cent = (1-alpha) exp(-T/T3) + alpha exp(-T/T1) + exp(-T2/T).  T3 and T1 must be non-zero
+     * (CRF_EINVAL otherwise); the Chemkin conventions T3 = 1e-30, T1 = 1e30 and a missing fourth
+     * parameter written as T2 = 1e30 or +inf are accepted (the terms evaluate to 0, alpha and 0). */
     const double *lnA0, *beta0, *Ea0_R, *alpha, *T3, *T1, *T2; /* [Nt] each */
 
     /* transport fits, natural-log cubics in ln T: ln f = c[0] + c[1] x + c[2] x^2 + c[3] x^3 */
@@ -95,7 +106,7 @@ typedef struct crf_mech crf_mech; /* opaque; owns the device copies of all table
 /* Builds the device-resident mechanism (tables re-laid-out for the kernels and uploaded to
  * the current CUDA device).  Returns CRF_EINVAL for inconsistent tables (bad version, species
  * index out of range, no reactant, W <= 0 ...), CRF_EUNSUPPORTED if Ns exceeds what the
- * kernels support (512), CRF_ECUDA on allocation failure.  *out is set only on success. */
+ * kernels support (CRF_MAX_SPECIES), CRF_ECUDA on allocation failure.  *out is set only on success. */
 int crf_mech_create(const crf_tables *tables, crf_mech **out);
 void crf_mech_destroy(crf_mech *mech);
 
@@ -138,20 +149,6 @@ int crf_mix_transport(const crf_mech *mech, const double *T, const double *p, co
  * bandwidth.  Synchronous: returns when every output is in host memory. */
 int crf_step_host(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
                   double *cp, double *h, double *omega, double *qdot, double *mu, double *lambda, double *rhoD);
-
-/* Sustained FP64 pipe rate of the current device: runs a register-only kernel of `iters`
- * dependent-chain DFMA groups on every SM and returns the FP64 instructions per second it
- * reached in *inst_per_s (the measured denominator of the ALU roofline).  Synchronous. */
-int crf_fp64_probe(int iters, double *inst_per_s);
-
-/* How many kernel launches this library has issued in this process (for bench.py). */
-int64_t crf_launch_count(void);
-
-/* Host-only diagnostic (no device needed): the tile schedule crf_mech_create lays out for crf_mix_transport on a
- * mechanism whose species fill nb blocks of 8, dealt to W warps.  Writes up to `cap` tiles as
- * int32 quadruples {round, kind (1 off-diagonal, 2 diagonal), jb, kb} to out and returns the number of tiles
- * of the schedule (which may exceed cap), or CRF_EINVAL. */
-int crf_transport_schedule(int nb, int W, int32_t *out, int cap);
 
 const char *crf_last_error(void);
 

@@ -16,10 +16,31 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcrf.so")
 _lib = None
 
+# include/crf.h (the method) and include/crf_diag.h (plan control, diagnostics)
 EXPORTS = ("crf_mech_create", "crf_mech_destroy", "crf_mech_set_stream", "crf_mech_num_species",
            "crf_mech_num_reactions", "crf_thermo", "crf_thermo_species", "crf_production_rates",
-           "crf_mix_transport", "crf_step_host", "crf_fp64_probe", "crf_launch_count", "crf_transport_schedule",
-           "crf_last_error")
+           "crf_mix_transport", "crf_step_host", "crf_last_error")
+EXPORTS_DIAG = ("crf_mech_create_ex", "crf_mech_plan_info", "crf_fp64_probe", "crf_launch_count",
+                "crf_transport_schedule")
+
+RATES_KERNELS = {"auto": 0, "generic": 1, "staged": 2, "group": 3, "thread": 4}
+TRANSPORT_KERNELS = {"auto": 0, "generic": 1, "small": 2, "tiled": 3}
+
+
+class PlanOptions(C.Structure):
+    """ctypes mirror of ``crf_plan_options`` (include/crf_diag.h)."""
+    _fields_ = [(n, C.c_int32) for n in ("rates_kernel", "rates_W", "rates_PPL", "rates_Rc", "transport_kernel",
+                                         "transport_W", "transport_PPL", "transport_panel")] \
+        + [("reserved", C.c_int32 * 8)]
+
+
+class PlanInfo(C.Structure):
+    """ctypes mirror of ``crf_plan_info`` (include/crf_diag.h)."""
+    _fields_ = [(n, C.c_int32) for n in ("rates_kernel", "rates_W", "rates_PPL", "rates_Rc", "rates_chunks",
+                                         "rates_stage_bytes", "rates_smem_bytes", "transport_kernel", "transport_W",
+                                         "transport_PPL", "transport_nb", "transport_stage_blocks",
+                                         "transport_stage_bytes", "transport_smem_bytes")] \
+        + [("reserved", C.c_int32 * 8)]
 
 
 class CrfError(RuntimeError):
@@ -36,6 +57,8 @@ def lib() -> C.CDLL:
         L = C.CDLL(LIB_PATH)
         vp, i64, dp = C.c_void_p, C.c_int64, C.c_void_p
         L.crf_mech_create.argtypes = [C.POINTER(packer.CrfTables), C.POINTER(vp)]
+        L.crf_mech_create_ex.argtypes = [C.POINTER(packer.CrfTables), C.POINTER(PlanOptions), C.POINTER(vp)]
+        L.crf_mech_plan_info.argtypes = [vp, C.POINTER(PlanInfo)]
         L.crf_mech_destroy.argtypes = [vp]
         L.crf_mech_destroy.restype = None
         L.crf_mech_set_stream.argtypes = [vp, vp]
@@ -86,15 +109,34 @@ def _host(t: torch.Tensor, shape):
 
 
 class Mechanism:
-    """Device-resident mechanism (``crf_mech``).  ``mech`` is a description dict or PackedTables."""
+    """Device-resident mechanism (``crf_mech``).  ``mech`` is a description dict or PackedTables.
+    ``options``: explicit kernel plan (``crf_plan_options``; kernels by name or number), default automatic."""
 
-    def __init__(self, mech):
+    def __init__(self, mech, options: dict | None = None):
         self.tables = mech if isinstance(mech, packer.PackedTables) else packer.pack(mech)
         self.Ns, self.Nr = self.tables.Ns, self.tables.Nr
         handle = C.c_void_p()
         struct = self.tables.as_struct()
-        _check(lib().crf_mech_create(C.byref(struct), C.byref(handle)))
+        if options:
+            o = dict(options)
+            if isinstance(o.get("rates_kernel"), str):
+                o["rates_kernel"] = RATES_KERNELS[o["rates_kernel"]]
+            if isinstance(o.get("transport_kernel"), str):
+                o["transport_kernel"] = TRANSPORT_KERNELS[o["transport_kernel"]]
+            po = PlanOptions(**o)
+            _check(lib().crf_mech_create_ex(C.byref(struct), C.byref(po), C.byref(handle)))
+        else:
+            _check(lib().crf_mech_create(C.byref(struct), C.byref(handle)))
         self._h = handle
+
+    def plan_info(self) -> dict:
+        """What this mechanism's calls will run (``crf_mech_plan_info``); kernels by name."""
+        info = PlanInfo()
+        _check(lib().crf_mech_plan_info(self._h, C.byref(info)))
+        d = {n: getattr(info, n) for n, _ in PlanInfo._fields_ if n != "reserved"}
+        d["rates_kernel"] = {v: k for k, v in RATES_KERNELS.items()}[d["rates_kernel"]]
+        d["transport_kernel"] = {v: k for k, v in TRANSPORT_KERNELS.items()}[d["transport_kernel"]]
+        return d
 
     def close(self):
         if getattr(self, "_h", None):

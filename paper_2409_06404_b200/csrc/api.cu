@@ -5,10 +5,11 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <new>
 #include <string>
 #include <vector>
 
-#include "../../include/crf.h"
+#include "../../include/crf_diag.h"
 #include "crf_internal.h"
 #include "host_plan.h"
 #include "launch.h"
@@ -38,6 +39,7 @@ void crf_count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 struct crf_mech {
     DevTables dev{};
+    crf_plan_info info{};
     void *block = nullptr;
     cudaStream_t stream = nullptr;
     // crf_step_host resources (lazy)
@@ -51,13 +53,16 @@ extern "C" {
 const char *crf_last_error(void) { return g_err.c_str(); }
 int64_t crf_launch_count(void) { return g_launches.load(); }
 
-int crf_mech_create(const crf_tables *t, crf_mech **out)
+}  // extern "C"
+
+namespace {
+
+int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out)
 {
-    if (!t || !out) return fail(CRF_EINVAL, "crf_mech_create: null argument");
     if (t->version != CRF_TABLES_VERSION) return fail(CRF_EINVAL, "crf_mech_create: tables version mismatch");
     const int Ns = t->Ns, Nr = t->Nr, N3 = t->N3, Nt = t->Nt;
     if (Ns < 1 || Nr < 0 || N3 < 0 || Nt < 0 || N3 + Nt > Nr) return fail(CRF_EINVAL, "crf_mech_create: bad counts");
-    if (Ns > 220) return fail(CRF_EUNSUPPORTED, "crf_mech_create: more than 220 species");
+    if (Ns > CRF_MAX_SPECIES) return fail(CRF_EUNSUPPORTED, "crf_mech_create: more than CRF_MAX_SPECIES (220) species");
     if (!(t->p_ref > 0.0)) return fail(CRF_EINVAL, "crf_mech_create: p_ref must be positive");
     const void *need[] = {t->W, t->Tmid, t->nasa_lo, t->nasa_hi, t->mu_c, t->lam_c, t->D_c};
     for (const void *q : need)
@@ -133,6 +138,9 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
         rT3.resize(Nt);
         rT1.resize(Nt);
         for (int i = 0; i < Nt; ++i) {
+            // (T3 = 1e-30 and T1 = T2 = 1e30 or inf are the Chemkin way of switching a term off: accepted)
+            if (!(t->T3[i] != 0.0) || !(t->T1[i] != 0.0) || std::isnan(t->T2[i]) || !std::isfinite(t->alpha[i]))
+                return fail(CRF_EINVAL, "crf_mech_create: Troe parameters: T3 and T1 must be non-zero, alpha finite");
             rT3[i] = 1.0 / t->T3[i];
             rT1[i] = 1.0 / t->T1[i];
         }
@@ -153,9 +161,26 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
                  oev = b.add(eff_val), olnA0 = b.add(lnA0), ob0 = b.add(beta0), oE0 = b.add(Ea0_R), oal = b.add(alpha),
                  orT3 = b.add(rT3), orT1 = b.add(rT1), oT2 = b.add(T2), omu = b.add(mu_c), olam = b.add(lam_c),
                  onD = b.add(nDc), owk = b.add(wilke), owq = b.add(wq);
-    const TransportPlanOffsets tpo = build_transport_plan(t, b);
-    const RatesPlanOffsets rpo = build_rates_plan(t, b);
-    const RatesSmemPlanOffsets rso = build_rates_smem_plan(t, b);
+    const TransportPlanOffsets tpo = build_transport_plan(t, opt, b);
+    const RatesPlanOffsets rpo = build_rates_plan(t, opt, b);
+    const RatesSmemPlanOffsets rso = build_rates_smem_plan(t, opt, b);
+    // what will run, and whether that is what was asked for
+    crf_plan_info info{};
+    info.rates_kernel = rso.W > 0 ? (rso.PPL == 4 ? CRF_RATES_THREAD : CRF_RATES_GROUP)
+                                  : (rpo.W > 0 ? CRF_RATES_STAGED : CRF_RATES_GENERIC);
+    if (rso.W > 0)
+        info.rates_W = rso.W, info.rates_PPL = rso.PPL, info.rates_Rc = rso.Rc, info.rates_chunks = rso.n_chunks,
+        info.rates_stage_bytes = rso.stage_bytes;
+    else if (rpo.W > 0)
+        info.rates_W = rpo.W, info.rates_PPL = 1, info.rates_Rc = rpo.Rc, info.rates_chunks = rpo.n_chunks;
+    info.transport_kernel = tpo.W > 0 ? CRF_TRANSPORT_TILED : (tpo.small_n > 0 ? CRF_TRANSPORT_SMALL : CRF_TRANSPORT_GENERIC);
+    if (tpo.W > 0)
+        info.transport_W = tpo.W, info.transport_PPL = tpo.PPL, info.transport_nb = tpo.nb,
+        info.transport_stage_blocks = tpo.n_wilke + tpo.n_rounds, info.transport_stage_bytes = tpo.stage_bytes;
+    if (opt.rates_kernel != CRF_RATES_AUTO && opt.rates_kernel != info.rates_kernel && Nr > 0)
+        return fail(CRF_EUNSUPPORTED, "crf_mech_create_ex: the requested rates kernel does not admit this mechanism");
+    if (opt.transport_kernel != CRF_TRANSPORT_AUTO && opt.transport_kernel != info.transport_kernel)
+        return fail(CRF_EUNSUPPORTED, "crf_mech_create_ex: the requested transport kernel does not admit this mechanism");
     crf_mech *mech = new (std::nothrow) crf_mech;
     if (!mech) return fail(CRF_ECUDA, "crf_mech_create: out of host memory");
     cudaError_t e = cudaMalloc(&mech->block, b.bytes.size());
@@ -185,7 +210,7 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
     d.mu_c = D(omu), d.lam_c = D(olam), d.nDc = D(onD), d.wilke_c = D(owk), d.wq = D(owq);
     TransportPlan &tp = d.tp;
     tp.W = tpo.W, tp.PPL = tpo.PPL, tp.NsP = tpo.NsP, tp.nb = tpo.nb, tp.n_wilke = tpo.n_wilke, tp.n_rounds = tpo.n_rounds;
-    tp.stage_bytes = tpo.stage_bytes, tp.dbg_skip = tpo.dbg_skip;
+    tp.stage_bytes = tpo.stage_bytes;
     tp.small = D(tpo.small), tp.small_n = tpo.small_n;
     tp.rounds = reinterpret_cast<const int4 *>(base + tpo.rounds);
     tp.pair_coef = base + tpo.pair_coef, tp.wilke_cP = D(tpo.wilke_cP), tp.sp = D(tpo.sp), tp.Ddiag = D(tpo.Ddiag);
@@ -202,7 +227,41 @@ int crf_mech_create(const crf_tables *t, crf_mech **out)
     rs.chunk = reinterpret_cast<const int4 *>(base + rso.chunk);
     rs.stage = base + rso.stage;
     rs.gco = D(rso.gco), rs.hco = D(rso.hco);
+    info.rates_smem_bytes = (int)rates_dynamic_smem(d);
+    info.transport_smem_bytes = (int)transport_dynamic_smem(d);
+    mech->info = info;
     *out = mech;
+    return CRF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int crf_mech_create_ex(const crf_tables *t, const crf_plan_options *options, crf_mech **out)
+{
+    if (!t || !out) return fail(CRF_EINVAL, "crf_mech_create: null argument");
+    crf_plan_options opt{};
+    if (options) opt = *options;
+    for (int32_t r : opt.reserved)
+        if (r != 0) return fail(CRF_EINVAL, "crf_mech_create_ex: reserved option fields must be 0");
+    try {  // the host re-layout allocates: no C++ exception may cross the boundary
+        return mech_create(t, opt, out);
+    } catch (const std::bad_alloc &) {
+        return fail(CRF_ECUDA, "crf_mech_create: out of host memory");
+    } catch (const std::exception &e) {
+        return fail(CRF_EINVAL, std::string("crf_mech_create: ") + e.what());
+    } catch (...) {
+        return fail(CRF_EINVAL, "crf_mech_create: unexpected exception");
+    }
+}
+
+int crf_mech_create(const crf_tables *t, crf_mech **out) { return crf_mech_create_ex(t, nullptr, out); }
+
+int crf_mech_plan_info(const crf_mech *mech, crf_plan_info *info)
+{
+    if (!mech || !info) return fail(CRF_EINVAL, "crf_mech_plan_info: null argument");
+    *info = mech->info;
     return CRF_OK;
 }
 
@@ -294,8 +353,12 @@ int crf_step_host(crf_mech *mech, const double *T, const double *p, const double
                 if (e != cudaSuccess) return fail_cuda(e, "crf_step_host: stream");
             }
             if (mech->pipe_buf[s]) cudaFree(mech->pipe_buf[s]);
+            mech->pipe_buf[s] = nullptr;  // (a failed cudaMalloc below must not leave a dangling pointer for crf_mech_destroy)
             e = cudaMalloc(&mech->pipe_buf[s], rows * chunk * sizeof(double));
-            if (e != cudaSuccess) return fail_cuda(e, "crf_step_host: cudaMalloc");
+            if (e != cudaSuccess) {
+                mech->pipe_buf[s] = nullptr;
+                return fail_cuda(e, "crf_step_host: cudaMalloc");
+            }
         }
         mech->pipe_chunk = chunk;
     }

@@ -15,7 +15,6 @@ struct TransportPlan {
     int W;         // warps per block (1, 2, 4 or 8); 0 = no plan (generic kernel)
     int PPL;       // points per lane (1 or 2)
     int NsP, nb;   // padded species count (multiple of 8) and number of 8-blocks
-    int dbg_skip;  // tuning only (CRF_TRANSPORT_SKIP): bit 0 skips the Wilke arithmetic, bit 1 the pair arithmetic
     int n_wilke;   // stage blocks of the Wilke phase (they come first in `rounds`)
     int n_rounds;  // stage blocks (rounds) of the pair phase
     int stage_bytes;          // largest stage block (multiple of 16)

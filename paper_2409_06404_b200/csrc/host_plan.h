@@ -6,7 +6,7 @@
 #include <cstring>
 #include <vector>
 
-#include "../../include/crf.h"
+#include "../../include/crf_diag.h"
 #include "crf_internal.h"
 
 struct BlockBuilder {
@@ -23,7 +23,7 @@ struct BlockBuilder {
 
 // Offsets (into the block) of what a plan points to; resolved to device pointers after the upload.
 struct TransportPlanOffsets {
-    int dbg_skip = 0, W = 0, PPL = 0, NsP = 0, nb = 0, n_wilke = 0, n_rounds = 0, stage_bytes = 0;
+    int W = 0, PPL = 0, NsP = 0, nb = 0, n_wilke = 0, n_rounds = 0, stage_bytes = 0;
     int small_n = 0;
     size_t small = 0, rounds = 0, pair_coef = 0, wilke_cP = 0, sp = 0, Ddiag = 0;
 };
@@ -37,6 +37,8 @@ struct RatesSmemPlanOffsets {
     size_t chunk = 0, stage = 0, gco = 0, hco = 0;
 };
 
-TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b);
-RatesPlanOffsets build_rates_plan(const crf_tables *t, BlockBuilder &b);
-RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b);
+// `opt` is the explicit plan request of crf_mech_create_ex (all zero = automatic); a builder that cannot honour
+// the request returns an empty plan (W = 0) and crf_mech_create_ex reports CRF_EUNSUPPORTED.
+TransportPlanOffsets build_transport_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b);
+RatesPlanOffsets build_rates_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b);
+RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b);

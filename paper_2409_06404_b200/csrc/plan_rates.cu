@@ -6,12 +6,16 @@
 #include "fastmath.cuh"
 #include "host_plan.h"
 
-RatesPlanOffsets build_rates_plan(const crf_tables *t, BlockBuilder &b)
+RatesPlanOffsets build_rates_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b)
 {
     RatesPlanOffsets o;
     const int Ns = t->Ns, Nr = t->Nr, N3 = t->N3, Nt = t->Nt, Ne = Nr - N3 - Nt;
     if (Ns > 128 || Nr == 0) return o;  // owned-species accumulators are registers: at most 32 per warp
-    const int W = Ns >= 32 ? 4 : (Ns >= 12 ? 2 : 1);
+    if (opt.rates_kernel != CRF_RATES_AUTO && opt.rates_kernel != CRF_RATES_STAGED) return o;
+    int W = Ns >= 32 ? 4 : (Ns >= 12 ? 2 : 1);
+    if (opt.rates_kernel == CRF_RATES_STAGED && (opt.rates_W == 1 || opt.rates_W == 2 || opt.rates_W == 4) &&
+        (Ns + opt.rates_W - 1) / opt.rates_W <= 32)
+        W = opt.rates_W;
     // q buffer rows: what is left of a third (W=4) of the SM's shared memory after the (C,g) state
     const size_t state = sizeof(double) * 2 * 32 * (size_t)(Ns + 1) + sizeof(double) * 32 * 2 * W;
     const size_t per_block = (227 * 1024) / (W == 4 ? 3 : (W == 2 ? 6 : 12)) - 1024;

@@ -3,7 +3,6 @@
 // the range check that admits the product form of the equilibrium constant.
 #include <cmath>
 #include <cstdint>
-#include <cstdlib>
 
 #include "fastmath.cuh"
 #include "host_plan.h"
@@ -150,20 +149,15 @@ std::vector<unsigned char> chunk_block(const Builder &B, const Chunk &ch, int PP
     return v;
 }
 
-int env_int(const char *name, int dflt)
-{
-    const char *s = std::getenv(name);
-    return s && *s ? std::atoi(s) : dflt;
-}
-
 }  // namespace
 
-RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
+RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b)
 {
     RatesSmemPlanOffsets o;
     Builder B{t, t->Ns, t->Nr, t->N3, t->Nt, t->Nr - t->N3 - t->Nt};
     const int Ns = B.Ns, Nr = B.Nr;
-    if (Nr == 0 || Ns > 256 || env_int("CRF_RATES_SMEM", 1) == 0) return o;
+    const int want = opt.rates_kernel;
+    if (Nr == 0 || Ns > 256 || want == CRF_RATES_STAGED || want == CRF_RATES_GENERIC) return o;
     for (int r = B.Ne; r < Nr; ++r)
         if (B.generic(r)) return o;  // a third body next to three explicit reactants: staged kernel
     if (!product_form_in_range(B)) return o;
@@ -174,9 +168,9 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
     // Small mechanisms: one THREAD per point (rates_thread_kernel in rates_smem.cu), 128 points per block, the (C, d)
     // state and omega as per-thread columns in shared memory (row stride 128 x 16 bytes = the layout of "4 points
     // per lane"), all chunk blocks resident at once.  Marked W = 1, PPL = 4; stage_bytes = all blocks.
-    // Default for Ns <= 12 (C2: 2.96 ms against 3.40 ms for the warp-group kernel); opt-in up to Ns = 24 with
-    // CRF_RATES_THREAD=1 (C3: 3.9 against 2.4 ms: the per-thread shared-memory chains are not hidden at 12 warps per SM).
-    if (Ns <= 24 && env_int("CRF_RATES_THREAD", Ns <= 12 ? 1 : 0) != 0 && env_int("CRF_RATES_W", 0) == 0) {
+    // Default for Ns <= 12 (C2: 2.96 ms against 3.40 ms for the warp-group kernel); on request (CRF_RATES_THREAD) up to
+    // Ns = 24 (C3: 3.9 against 2.4 ms: the per-thread shared-memory chains are not hidden at 12 warps per SM).
+    if (Ns <= 24 && (want == CRF_RATES_THREAD || (want == CRF_RATES_AUTO && Ns <= 12 && opt.rates_W == 0))) {
         chunks = make_chunks(B, Nr);
         for (const Chunk &ch : chunks) {
             blocks.push_back(chunk_block(B, ch, 4, 1, 4));
@@ -184,10 +178,11 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
         }
         if (stage_bytes <= 24 * 1024) o.W = 1, o.PPL = 4, o.maxown = 4, o.Rc = 0;
     }
+    if (want == CRF_RATES_THREAD && o.W == 0) return o;  // unsupported request
     if (o.W == 0) {
     // warps per point group W and points per lane PPL: 16 warps per SM, so a block may use 1/(16/W) of the
     // SM's shared memory; the (C, d) state of its 32 PPL points should leave room for the q buffer and the
-    // two chunk blocks.  CRF_RATES_W / CRF_RATES_PPL / CRF_RATES_RC override (tuning).
+    // two chunk blocks.  crf_plan_options.rates_W / rates_PPL / rates_Rc override.
     auto budget = [](int W) { return (size_t)233472 / (16 / W) - 1024; };
     auto state = [&](int PPL) { return (size_t)(Ns + 1) * 512 * PPL; };
     // Measured (rates, ms): C5 W/PPL 16/2 11.0, 8/1 13.8, 16/1 14.4; C4 8/2 9.0, 16/2 10.9, 8/1 13.0, 4/2 21.0;
@@ -198,15 +193,15 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, BlockBuilder &b)
             if (state(ppl) <= budget(w) * 6 / 10 && (Ns + w - 1) / w <= 16) return w;
         return 0;
     };
-    int PPL = env_int("CRF_RATES_PPL", pick_w(2) ? 2 : 1);
+    int PPL = opt.rates_PPL ? opt.rates_PPL : (pick_w(2) ? 2 : 1);
     if (PPL != 1 && PPL != 2) PPL = 1;
-    int W = env_int("CRF_RATES_W", 0);
+    int W = opt.rates_W;
     if (W != 4 && W != 8 && W != 16) W = pick_w(PPL) ? pick_w(PPL) : 16;
     if ((Ns + W - 1) / W > 16 || state(PPL) + 2 * W * 256 * PPL > budget(W)) return o;
 
     const int own = (Ns + W - 1) / W, maxown = own <= 4 ? 4 : (own <= 8 ? 8 : 16);
     const int step = 2 * W;
-    int Rc = env_int("CRF_RATES_RC", 0);
+    int Rc = opt.rates_Rc;
     for (int cand = Rc > 0 ? (Rc + step - 1) / step * step : std::min(256, (Nr + step - 1) / step * step);
          cand >= step; cand -= step) {
         chunks = make_chunks(B, cand);

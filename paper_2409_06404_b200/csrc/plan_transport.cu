@@ -2,7 +2,6 @@
 // transport_tiled.cu (see the header comment there and TransportPlan in crf_internal.h).
 #include <cmath>
 #include <cstdint>
-#include <cstdlib>
 
 #include "fastmath.cuh"
 #include "host_plan.h"
@@ -12,12 +11,6 @@ namespace {
 struct Tile {
     int kind, jb, kb;  // kind 1: off-diagonal tile (jb < kb), 2: diagonal tile (jb = kb)
 };
-
-int env_int(const char *name, int dflt)
-{
-    const char *s = std::getenv(name);
-    return s && *s ? std::atoi(s) : dflt;
-}
 
 // Rounds of at most W tiles whose species blocks are pairwise disjoint: the circle method of a round-robin
 // tournament over the nb blocks (an odd nb gets a dummy block; meeting the dummy is the block's bye, in
@@ -54,12 +47,14 @@ std::vector<std::vector<Tile>> schedule_rounds(int nb, int W)
 
 }  // namespace
 
-TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
+TransportPlanOffsets build_transport_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b)
 {
     TransportPlanOffsets o;
     const int Ns = t->Ns;
+    const int want = opt.transport_kernel;
+    if (want == CRF_TRANSPORT_GENERIC) return o;
     if (Ns < 17) {  // small mechanisms: the register-resident kernel (transport_small.cu), one flat table
-        if (Ns < 2 || env_int("CRF_TRANSPORT_SMALL", 1) == 0) return o;  // generic kernel
+        if (Ns < 2 || want == CRF_TRANSPORT_TILED) return o;  // generic kernel (or an unsupported request)
         const int npair = Ns * (Ns + 1) / 2;
         auto pidx = [&](int j, int k) { return j * Ns - (j * (j - 1)) / 2 + (k - j); };  // j <= k
         std::vector<double> tb;
@@ -84,22 +79,21 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
         o.small = b.add(tb);
         return o;
     }
+    if (want == CRF_TRANSPORT_SMALL) return o;  // unsupported request: Ns > 16
     const int nb = (Ns + 7) / 8, NsP = 8 * nb;
     // warps per point group: one per tile of a round-robin round (nb odd: (nb+1)/2, nb even: nb/2), at most 8;
     // points per lane: 1 (16 warps per SM at 128 registers) or 2 (8 warps per SM, every coefficient load
-    // serves two points).  CRF_TRANSPORT_W / CRF_TRANSPORT_PPL override (tuning).
+    // serves two points).  crf_plan_options.transport_W / transport_PPL override.
     const int per_round = std::max(1, (nb + (nb & 1)) / 2);
-    int W = env_int("CRF_TRANSPORT_W", 0);
+    int W = opt.transport_W;
     if (W != 1 && W != 2 && W != 4 && W != 8) {
         W = 1;
         while (W < 8 && W < per_round) W *= 2;
         if (nb <= 3) W = 1;  // a round of nb = 3 is one full tile and one diagonal tile: two warps would idle 28 %
                              // (C3: W = 1 3.0 ms, W = 2 4.1 ms); the state is small, so the SM still holds 16 blocks
     }
-    int PPL = env_int("CRF_TRANSPORT_PPL", 1);
-    if (PPL != 1 && PPL != 2) PPL = 1;
+    const int PPL = opt.transport_PPL == 2 ? 2 : 1;
     o.W = W, o.PPL = PPL, o.NsP = NsP, o.nb = nb;
-    o.dbg_skip = env_int("CRF_TRANSPORT_SKIP", 0);
 
     const int npair = Ns * (Ns + 1) / 2;
     auto pair_index = [&](int j, int k) {
@@ -126,8 +120,8 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, BlockBuilder &b)
     };
     // Wilke stage blocks: pass p covers the row blocks p W .. p W + W - 1 (one per warp), a panel covers up to
     // kPanel column blocks (as many as keep the block within 20 KB: fewer, larger stage steps measured faster, C5 panel
-    // 3 -> 5 29.2 -> 28.8 ms, C4 15.5 -> 15.0 ms; CRF_TRANSPORT_PANEL overrides); payload [W][8 rows][8 nJ columns] of c_kj (0 in padded rows/columns)
-    const int kPanel = std::max(1, env_int("CRF_TRANSPORT_PANEL", std::min({nb, 5, 20480 / (W * 512)}))), npass = (nb + W - 1) / W;
+    // 3 -> 5 29.2 -> 28.8 ms, C4 15.5 -> 15.0 ms; crf_plan_options.transport_panel overrides); payload [W][8 rows][8 nJ columns] of c_kj (0 in padded rows/columns)
+    const int kPanel = opt.transport_panel > 0 ? std::min(opt.transport_panel, nb) : std::max(1, std::min({nb, 5, 20480 / (W * 512)})), npass = (nb + W - 1) / W;
     for (int ps = 0; ps < npass; ++ps)
         for (int J0 = 0; J0 < nb; J0 += kPanel) {
             const int nJ = std::min(kPanel, nb - J0);

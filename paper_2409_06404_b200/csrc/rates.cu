@@ -146,6 +146,14 @@ cudaError_t launch_b(const DevTables &m, const double *T, const double *p, const
 
 }  // namespace
 
+size_t rates_dynamic_smem(const DevTables &m)
+{
+    if (m.rs.W > 0) return rates_smem_dynamic_smem(m);
+    if (m.rp.W > 0) return rates_staged_dynamic_smem(m);
+    const size_t per_thread = sizeof(double) * 2 * (size_t)m.Ns;
+    return per_thread * (per_thread * 128 <= 100 * 1024 ? 128 : (per_thread * 64 <= 200 * 1024 ? 64 : 32));
+}
+
 cudaError_t launch_rates(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                          double *omega, double *qdot, cudaStream_t st)
 {

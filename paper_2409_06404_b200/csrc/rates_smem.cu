@@ -129,8 +129,10 @@ __device__ __forceinline__ void reaction_q(const char *blk, const char *rec, con
             const double y0 = fma(t01.y, c.L[u], fma(t23.x, c.rT[u], t01.x));
             const double l2Pr = (y0 - yinf) + log2_fast(fmax(M[u], 1.0e-300));  // log2(k_0 [M] / k_inf)
             const double al = t23.y;
-            const double Fc = fma(1.0 - al, exp2c(c.T[u] * t45.x),
-                                  fma(al, exp2c(c.T[u] * t45.y), exp2c(t67.x * c.rT[u])));
+            // (the arguments are clamped BEFORE the range reduction: Chemkin-style switched-off terms, T3 = 1e-30 or
+            // T2 = 1e30 / inf, give arguments of -1e33 or -inf, whose integer part has no meaning as an exponent)
+            const double Fc = fma(1.0 - al, exp2c(fmax(c.T[u] * t45.x, -1022.0)),
+                                  fma(al, exp2c(fmax(c.T[u] * t45.y, -1022.0)), exp2c(fmax(t67.x * c.rT[u], -1022.0))));
             const double l2Fc = log2_fast(fmax(Fc, 1.0e-300));
             const double l10_2 = 0.30102999566398119521;
             const double lFc = l10_2 * l2Fc;
@@ -417,7 +419,7 @@ template <int W, int PPL, int MAXOWN>
 cudaError_t launch_k(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
                      double *qdot, cudaStream_t st)
 {
-    const size_t smem = (size_t)(m.Ns + 1) * 512 * PPL + (size_t)m.rs.Rc * 256 * PPL + 2 * (size_t)m.rs.stage_bytes;
+    const size_t smem = rates_smem_dynamic_smem(m);
     cudaError_t e = cudaFuncSetAttribute(rates_smem_kernel<W, PPL, MAXOWN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem);
     if (e != cudaSuccess) return e;
@@ -595,7 +597,7 @@ __global__ void __launch_bounds__(RT_B) rates_thread_kernel(DevTables m, const d
 cudaError_t launch_thread(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
                           double *qdot, cudaStream_t st)
 {
-    const size_t smem = (size_t)(m.Ns + 1) * (2048 + 1024) + (size_t)m.rs.stage_bytes + 256 * (size_t)m.Ns;
+    const size_t smem = rates_smem_dynamic_smem(m);
     cudaError_t e = cudaFuncSetAttribute(rates_thread_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     rates_thread_kernel<<<(unsigned)((n + RT_B - 1) / RT_B), RT_B, smem, st>>>(m, T, p, Y, n, omega, qdot);
@@ -604,6 +606,13 @@ cudaError_t launch_thread(const DevTables &m, const double *T, const double *p, 
 }
 
 }  // namespace
+
+size_t rates_smem_dynamic_smem(const DevTables &m)
+{
+    if (m.rs.W == 1)  // thread kernel: state + omega columns, all chunk blocks, g and h sets
+        return (size_t)(m.Ns + 1) * (2048 + 1024) + (size_t)m.rs.stage_bytes + 256 * (size_t)m.Ns;
+    return (size_t)(m.Ns + 1) * 512 * m.rs.PPL + (size_t)m.rs.Rc * 256 * m.rs.PPL + 2 * (size_t)m.rs.stage_bytes;
+}
 
 cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                               double *omega, double *qdot, cudaStream_t st)

@@ -104,7 +104,9 @@ __device__ __forceinline__ double reaction_q(const DevTables &m, const char *sCG
     const double y0 = fma(t01.y, c.L, fma(t23.x, c.rT, t01.x));
     const double Pr = exp2_clamped(y0 - yinf) * M;
     const double al = t23.y;
-    const double Fc = fma(1.0 - al, exp2_clamped(c.Ti * t45.x), fma(al, exp2_clamped(c.Ti * t45.y), exp2_clamped(t67.x * c.rT)));
+    // (arguments clamped before the range reduction: T3 = 1e-30, T2 = 1e30 or inf switch a term off, rates_smem.cu)
+    const double Fc = fma(1.0 - al, exp2_clamped(fmax(c.Ti * t45.x, -1022.0)),
+                          fma(al, exp2_clamped(fmax(c.Ti * t45.y, -1022.0)), exp2_clamped(fmax(t67.x * c.rT, -1022.0))));
     const double lFc = log10(fmax(Fc, 1.0e-300));
     const double lPr = log10(Pr);
     const double cc = -0.4 - 0.67 * lFc;
@@ -257,7 +259,7 @@ template <int W, int MAXOWN>
 cudaError_t launch_wm(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
                       double *qdot, cudaStream_t st)
 {
-    const size_t smem = sizeof(double) * (2 * 32 * (size_t)(m.Ns + 1) + 32 * (size_t)m.rp.Rc + 2 * W * 32);
+    const size_t smem = rates_staged_dynamic_smem(m);
     cudaError_t e = cudaFuncSetAttribute(rates_staged_kernel<W, MAXOWN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem);
     if (e != cudaSuccess) return e;
@@ -277,6 +279,11 @@ cudaError_t launch_w(const DevTables &m, const double *T, const double *p, const
 }
 
 }  // namespace
+
+size_t rates_staged_dynamic_smem(const DevTables &m)
+{
+    return sizeof(double) * (2 * 32 * (size_t)(m.Ns + 1) + 32 * (size_t)m.rp.Rc + 2 * (size_t)m.rp.W * 32);
+}
 
 cudaError_t launch_rates_staged(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                                 double *omega, double *qdot, cudaStream_t st)

@@ -107,6 +107,14 @@ cudaError_t launch_b(const DevTables &m, const double *T, const double *Y, int64
 
 }  // namespace
 
+size_t transport_dynamic_smem(const DevTables &m)
+{
+    if (m.tp.W > 0) return transport_tiled_dynamic_smem(m);
+    if (m.tp.small_n > 0) return transport_small_dynamic_smem(m);
+    const size_t per_thread = sizeof(double) * 4 * (size_t)m.Ns;
+    return per_thread * (per_thread * 128 <= 100 * 1024 ? 128 : (per_thread * 64 <= 200 * 1024 ? 64 : 32));
+}
+
 cudaError_t launch_transport(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                              double *mu, double *lambda, double *rhoD, cudaStream_t st)
 {

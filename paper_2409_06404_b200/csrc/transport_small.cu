@@ -114,13 +114,15 @@ template <int NS>
 cudaError_t launch_ns(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu, double *lambda,
                       double *rhoD, cudaStream_t st)
 {
-    const size_t smem = sizeof(double) * ((size_t)m.tp.small_n + 64);
+    const size_t smem = transport_small_dynamic_smem(m);
     transport_small_kernel<NS><<<(unsigned)((n + TBS - 1) / TBS), TBS, smem, st>>>(m, T, Y, n, mu, lambda, rhoD);
     crf_count_launch();
     return cudaGetLastError();
 }
 
 }  // namespace
+
+size_t transport_small_dynamic_smem(const DevTables &m) { return sizeof(double) * ((size_t)m.tp.small_n + 64); }
 
 cudaError_t launch_transport_small(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu,
                                    double *lambda, double *rhoD, cudaStream_t st)

@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
             cur = *reinterpret_cast<const int4 *>(blk);
             stage_async(sStage + (size_t)((s + 1) & 1) * tp.stage_bytes, tp.pair_coef + cur.x, cur.y, threadIdx.x, 32 * W);
             const int J0 = ds.z & 0xff, I = ((ds.z >> 8) & 0xff) * W + warp, nJ = ds.w;
-            if (I >= nb || (tp.dbg_skip & 1)) continue;
+            if (I >= nb) continue;
             if (ds.z & (1 << 16)) {
 #pragma unroll
                 for (int u = 0; u < PPL; ++u)
@@ -341,8 +341,7 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
         const int2 d = *reinterpret_cast<const int2 *>(blk + 16 + 8 * warp);
         const int kind = d.x & 0xff, jb = (d.x >> 8) & 0xff, kb = (d.x >> 16) & 0xff;
         const double2 *cf = reinterpret_cast<const double2 *>(blk + d.y);
-        if (tp.dbg_skip & 2) {
-        } else if (kind == 1)
+        if (kind == 1)
             tile_offdiag<PPL>(cf, L, sZl, sSl, jb, kb, sTab);
         else if (kind == 2)
             tile_diag<PPL>(cf, L, sZl, sSl, jb, sTab);
@@ -382,7 +381,7 @@ template <int W, int PPL>
 cudaError_t launch_w(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu, double *lambda,
                      double *rhoD, cudaStream_t st)
 {
-    const size_t smem = sizeof(double) * ((size_t)2 * m.tp.NsP + 4 * W) * PPL * 32 + 2 * (size_t)m.tp.stage_bytes;
+    const size_t smem = transport_tiled_dynamic_smem(m);
     cudaError_t e = cudaFuncSetAttribute(transport_tiled_kernel<W, PPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem);
     if (e != cudaSuccess) return e;
@@ -394,6 +393,11 @@ cudaError_t launch_w(const DevTables &m, const double *T, const double *Y, int64
 }
 
 }  // namespace
+
+size_t transport_tiled_dynamic_smem(const DevTables &m)
+{
+    return sizeof(double) * ((size_t)2 * m.tp.NsP + 4 * (size_t)m.tp.W) * m.tp.PPL * 32 + 2 * (size_t)m.tp.stage_bytes;
+}
 
 cudaError_t launch_transport_tiled(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu,
                                    double *lambda, double *rhoD, cudaStream_t st)

@@ -37,7 +37,9 @@ def evaluate(mech, T, p, Y):
     g = [t[1] - t[2] for t in th]
     hmol = [t[1] * R * T for t in th]
     out = dict(cp=sum(Y[k] * th[k][0] * R / W[k] for k in range(ns)),
-               h=sum(Y[k] * hmol[k] / W[k] for k in range(ns)))
+               h=sum(Y[k] * hmol[k] / W[k] for k in range(ns)),
+               h_scale=sum(abs(Y[k] * hmol[k] / W[k]) for k in range(ns)),
+               rho=rho, Wbar=Wbar, cpk=[t[0] * R for t in th], hk=hmol)
     omega = [mp.mpf(0)] * ns
     S = [mp.mpf(0)] * ns
     pref = mp.mpf(float(mech["p_ref"]))

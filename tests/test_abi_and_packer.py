@@ -15,6 +15,7 @@ from tests.helpers import rxn, tiny_mech
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "crf.h")
+HEADER_DIAG = os.path.join(ROOT, "include", "crf_diag.h")
 
 
 @pytest.fixture(scope="module")
@@ -22,8 +23,8 @@ def lib_path():
     return build.build()
 
 
-def _declared_functions():
-    src = open(HEADER).read()
+def _declared_functions(path=HEADER):
+    src = open(path).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(crf_[a-z0-9_]+)\s*\(", src)))
 
@@ -35,6 +36,33 @@ def test_library_exports_every_declared_symbol(lib_path):
     for nm in names:
         assert hasattr(L, nm), f"libcrf.so does not export {nm}"
     assert sorted(binding.EXPORTS) == names, "binding.EXPORTS and include/crf.h disagree"
+    diag = _declared_functions(HEADER_DIAG)
+    for nm in diag:
+        assert hasattr(L, nm), f"libcrf.so does not export {nm} (crf_diag.h)"
+    assert sorted(binding.EXPORTS_DIAG) == diag, "binding.EXPORTS_DIAG and include/crf_diag.h disagree"
+    # the method header holds the method only: no probe, counter or schedule dump
+    assert not {"crf_fp64_probe", "crf_launch_count", "crf_transport_schedule"} & set(names)
+
+
+def test_plan_structs_mirror_header():
+    src = re.sub(r"/\*.*?\*/", "", open(HEADER_DIAG).read(), flags=re.S)
+    for cname, mirror in (("crf_plan_options", binding.PlanOptions), ("crf_plan_info", binding.PlanInfo)):
+        body = re.search(r"typedef struct %s \{(.*?)\} %s;" % (cname, cname), src, flags=re.S).group(1)
+        fields = []
+        for decl in body.split(";"):
+            decl = decl.strip()
+            if decl:
+                fields += [w.strip(",").split("[")[0] for w in decl.split()[1:]]
+        assert fields == [f[0] for f in mirror._fields_], cname
+
+
+def test_no_environment_tuning_in_the_library():
+    """Kernel plans are chosen from the mechanism or requested through crf_plan_options: libcrf.so reads no
+    environment variable and carries no work-skipping switch."""
+    csrc = os.path.join(ROOT, "paper_2409_06404_b200", "csrc")
+    for f in os.listdir(csrc):
+        text = open(os.path.join(csrc, f)).read()
+        assert "getenv" not in text and "dbg_skip" not in text and "_SKIP" not in text, f
 
 
 def test_argument_errors_need_no_gpu(lib_path):

@@ -441,7 +441,10 @@ def test_against_mpmath(Oracle, which):
     for i in range(st["T"].size):
         ref = mp_reference.evaluate(m, st["T"][i], st["p"][i], st["Y"][:, i])
         assert abs(th["cp"][i] - ref["cp"]) <= 1e-14 * abs(ref["cp"])
-        assert abs(th["h"][i] - ref["h"]) <= 1e-14 * th["h_scale"][i]
+        # the two tolerance scales the GPU parity tests divide by (tests/parity.py) are themselves pinned
+        assert abs(th["h_scale"][i] - ref["h_scale"]) <= 1e-12 * ref["h_scale"]
+        assert abs(r["S_q"][i] - ref["S_q"]) <= 1e-12 * ref["S_q"]
+        assert abs(th["h"][i] - ref["h"]) <= 1e-14 * ref["h_scale"]
         for k in range(len(m["W"])):
             assert abs(r["omega"][k, i] - ref["omega"][k]) <= 2e-13 * ref["S_omega"][k] + 1e-300, (i, k)
             assert abs(r["S_omega"][k, i] - ref["S_omega"][k]) <= 1e-12 * ref["S_omega"][k]

@@ -205,31 +205,161 @@ def test_fp64_probe(binding):
 
 
 PLAN_OVERRIDES = [
-    {"CRF_TRANSPORT_PPL": "2"},                        # two points per lane in the tiled transport kernel
-    {"CRF_TRANSPORT_W": "4"},                          # rounds split over fewer warps than tiles
-    {"CRF_TRANSPORT_W": "1", "CRF_TRANSPORT_PPL": "2"},
-    {"CRF_RATES_W": "8", "CRF_RATES_PPL": "1"},
-    {"CRF_RATES_W": "4", "CRF_RATES_PPL": "2", "CRF_RATES_RC": "32"},   # many small chunks
-    {"CRF_RATES_SMEM": "0"},                           # the staged fallback kernel
-    {"CRF_RATES_THREAD": "1"},                         # one thread per point (default for Ns <= 12; C3 here)
-    {"CRF_RATES_THREAD": "0"},                         # ... and the warp-group kernel where that is the default (C2)
-    {"CRF_TRANSPORT_SMALL": "0"},                      # generic transport kernel (only differs for Ns <= 16)
+    dict(transport_kernel="tiled", transport_PPL=2),       # two points per lane in the tiled transport kernel
+    dict(transport_kernel="tiled", transport_W=4),         # rounds split over fewer warps than tiles
+    dict(transport_kernel="tiled", transport_W=1, transport_PPL=2),
+    dict(transport_kernel="tiled", transport_panel=1),     # one column block per Wilke panel (most stage steps)
+    dict(rates_kernel="group", rates_W=8, rates_PPL=1),
+    dict(rates_kernel="group", rates_W=4, rates_PPL=2, rates_Rc=32),   # many small chunks
+    dict(rates_kernel="group", rates_W=16, rates_PPL=2),
+    dict(rates_kernel="staged"),                           # log-space K_c kernel (the automatic fall-back)
+    dict(rates_kernel="generic"),                          # one thread per point, libm
+    dict(rates_kernel="thread"),                           # one thread per point, product form (default for Ns <= 12)
+    dict(transport_kernel="generic"),
+    dict(transport_kernel="small"),
 ]
 
 
-@pytest.mark.parametrize("env", PLAN_OVERRIDES, ids=lambda e: ",".join(f"{k[4:]}={v}" for k, v in e.items()))
+def _admits(name, opt):
+    Ns = wl.CONFIGS[name]["Ns"]
+    if opt.get("rates_kernel") == "thread" and Ns > 24:
+        return False
+    if opt.get("rates_kernel") == "group" and opt.get("rates_W") and (Ns + opt["rates_W"] - 1) // opt["rates_W"] > 16:
+        return False
+    if opt.get("transport_kernel") == "small" and Ns > 16:
+        return False
+    if opt.get("transport_kernel") == "tiled" and Ns < 17:
+        return False
+    return True
+
+
+@pytest.mark.parametrize("opt", PLAN_OVERRIDES, ids=lambda o: ",".join(f"{k}={v}" for k, v in o.items()))
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
-def test_plan_overrides(binding, oracle_mod, monkeypatch, name, env):
-    """The kernel plans are chosen in crf_mech_create; the CRF_* tuning overrides select the other template
-    instances (warps per point group, points per lane, chunk size, fallback kernel): each must meet the same
-    tolerances on a ragged size."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+def test_plan_overrides(binding, oracle_mod, name, opt):
+    """The kernel plans are chosen in crf_mech_create; crf_mech_create_ex (crf_diag.h) selects the other kernels and
+    template instances (warps per point group, points per lane, chunk size, fall-back kernels): each must meet the
+    same tolerances on a ragged size, and a request the mechanism does not admit must fail, not fall back."""
     desc = wl.make_mechanism(name)
-    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    if not _admits(name, opt):
+        with pytest.raises(binding.CrfError):
+            binding.Mechanism(desc, options=opt)
+        return
+    try:
+        gm = binding.Mechanism(desc, options=opt)
+    except binding.CrfError as err:
+        # an explicit warps-per-group request may not fit the shared-memory budget of this mechanism: refused, never
+        # silently replaced (which kernel ran is asserted below for every request that is honoured)
+        assert "does not admit" in str(err) and opt.get("rates_W"), (opt, err)
+        return
+    om = oracle_mod.Oracle(desc)
+    info = gm.plan_info()
+    for k, v in opt.items():
+        if k not in ("rates_Rc", "transport_panel"):
+            assert info[k] == v, (k, info)
     n = SMALL_N[name] + 2
     st = wl.make_state(name, n=n, total=n)
-    parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), f"{name} {env} n={n}")
+    parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), f"{name} {opt} n={n}")
+
+
+BIG = {"Ns160": dict(seed=5, elements=("C", "H", "O", "N"), Ns=160, Nr=900, N3=60, Nt=40, ndup=0, cmax=3, eff_all=False),
+       "Ns220": dict(seed=6, elements=("C", "H", "O", "N"), Ns=220, Nr=1200, N3=80, Nt=60, ndup=6, cmax=3, eff_all=False)}
+
+
+@pytest.mark.parametrize("which", ["Ns160", "Ns220"])
+def test_mechanisms_larger_than_C5(binding, oracle_mod, which):
+    """crf_mech_create accepts up to CRF_MAX_SPECIES = 220 species: above C5 (118) the rates plan runs under a
+    tighter shared-memory budget (one point per lane, more chunks) and the tiled transport kernel has up to 28
+    species blocks.  Same tolerances, ragged size; the automatic plan must be a fast kernel, not the generic one."""
+    desc = wl.make_mechanism(None, **BIG[which])
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    info = gm.plan_info()
+    assert info["rates_kernel"] == "group" and info["transport_kernel"] == "tiled", info
+    n = 3 * 64 + 37
+    st = wl.make_state("C5", n=n, Ns=BIG[which]["Ns"])
+    parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), f"{which} n={n} {info}")
+    with pytest.raises(binding.CrfError):  # one species more than the limit
+        binding.Mechanism(wl.make_mechanism(None, **dict(BIG["Ns220"], Ns=221)))
+
+
+def _far_from_equilibrium_mechanism():
+    """Formation enthalpies so far apart that the product form of 1/K_c (numerator and denominator formed
+    separately) would leave the double range at the cold end of the validated window: the two reactants sit
+    1.2e5 K (1000 kJ/mol) above the products, so at 250 K the numerator alone is 2^1385."""
+    from tests.helpers import const_cp_nasa
+    W = [10.0, 12.0, 9.0, 13.0, 28.0]
+    nasa = np.array([const_cp_nasa(3.5, 1.2e5, 4.0), const_cp_nasa(4.0, 1.2e5, 5.0), const_cp_nasa(3.8, 0.0, 6.0),
+                     const_cp_nasa(4.2, -2.0e3, 3.0), const_cp_nasa(3.5, 0.0, 5.0)])
+    rx = [rxn([(0, 1), (1, 1)], [(2, 1), (3, 1)], A=1e12, beta=0.5, Ea=10.0),
+          rxn([(0, 2)], [(2, 1), (3, 1)], A=1e10, beta=0.0, Ea=30.0, type="three_body", eff={4: 2.0}),
+          rxn([(2, 1), (3, 1)], [(1, 2)], A=1e9, beta=1.0, Ea=5.0)]   # the same gap uphill: K_c underflows towards 0
+    return tiny_mech(W, rx, nasa=(nasa, nasa))
+
+
+def test_automatic_fallback_to_log_space_kernel(binding, oracle_mod):
+    """No option is passed: crf_mech_create itself must notice that the product form of K_c is out of range and pick
+    the log-space kernel (rates_staged.cu); requesting the product-form kernels for this mechanism must fail."""
+    desc = _far_from_equilibrium_mechanism()
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    assert gm.plan_info()["rates_kernel"] == "staged", gm.plan_info()
+    for kernel in ("group", "thread"):
+        with pytest.raises(binding.CrfError):
+            binding.Mechanism(desc, options=dict(rates_kernel=kernel))
+    rng = np.random.default_rng(8)
+    n = 333
+    # (reaction 3 runs uphill by the same gap: its K_c is 1e-100 at 1000 K, so k_r = k_f/K_c is huge but finite
+    # above ~700 K; below that the oracle's own K_c underflows to 0 and the definition gives inf - not a test case)
+    st = dict(T=rng.uniform(800.0, 2500.0, n), p=rng.uniform(5e4, 5e6, n),
+              Y=np.ascontiguousarray(rng.dirichlet(np.ones(5), size=n).T))
+    ref = parity.run_oracle(om, st)
+    assert np.all(np.isfinite(ref["omega"]))
+    parity.assert_parity(parity.run_gpu(gm, st), ref, "far from equilibrium (automatic staged kernel)")
+    gg = binding.Mechanism(desc, options=dict(rates_kernel="generic"))
+    parity.assert_parity(parity.run_gpu(gg, st), ref, "far from equilibrium (generic kernel)")
+
+
+def test_mechanism_without_reactions(binding, oracle_mod):
+    """Nr = 0 (a transport/thermo-only mechanism): no rates plan exists, crf_production_rates runs the generic kernel
+    and returns exact zeros."""
+    desc = tiny_mech([2.0, 32.0, 18.0, 28.0], [])
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    assert gm.plan_info()["rates_kernel"] == "generic"
+    rng = np.random.default_rng(2)
+    n = 97
+    st = dict(T=rng.uniform(300, 2500, n), p=np.full(n, P_REF), Y=np.ascontiguousarray(rng.dirichlet(np.ones(4), size=n).T))
+    gpu = parity.run_gpu(gm, st)
+    assert np.all(gpu["omega"] == 0.0) and np.all(gpu["qdot"] == 0.0)
+    parity.assert_parity(gpu, parity.run_oracle(om, st), "Nr = 0")
+
+
+TROE_SETS = {
+    "chemkin_3_parameter": dict(alpha=0.5, T3=1e-30, T1=1e30, T2=1e30),      # 'TROE/0.5 1E-30 1E30/' + missing T2
+    "T2_infinite": dict(alpha=0.7, T3=150.0, T1=1800.0, T2=float("inf")),
+    "T2_huge": dict(alpha=0.62, T3=1e-30, T1=900.0, T2=1e300),
+    "lindemann_inside_troe": dict(alpha=1.0, T3=1e300, T1=1e300, T2=1e300),  # F_cent = 1 -> F = 1
+    "T3_infinite": dict(alpha=0.4, T3=float("inf"), T1=700.0, T2=4000.0),
+}
+
+
+@pytest.mark.parametrize("kernel", ["auto", "group", "staged", "generic", "thread"])
+@pytest.mark.parametrize("which", sorted(TROE_SETS))
+def test_troe_switched_off_terms(binding, oracle_mod, which, kernel):
+    """Chemkin mechanisms switch Troe terms off with T3 = 1e-30, T1 = 1e30 and a missing (or 1e30 / infinite) T2:
+    the arguments of the three exponentials of F_cent then reach -1e33 or -inf.  Every rates kernel must return what
+    the definition gives (the terms are 0, alpha and 0) instead of reading garbage exponent bits."""
+    W = [2.0, 32.0, 34.0, 17.0, 28.0]
+    troe = dict(A0=3e17, beta0=-0.8, Ea0=2.0, **TROE_SETS[which])
+    rx = [rxn([(3, 2)], [(2, 1)], A=2e13, beta=-0.3, Ea=1.0, type="falloff", eff={0: 2.0, 4: 0.7}, troe=troe),
+          rxn([(0, 1), (1, 1)], [(3, 2)], A=1e11, beta=0.5, Ea=60.0),
+          rxn([(3, 1), (0, 1)], [(2, 1)], A=5e12, beta=0.0, Ea=8.0, type="falloff", eff={}, troe=dict(troe, A0=1e16))]
+    desc = tiny_mech(W, rx)
+    gm, om = binding.Mechanism(desc, options=dict(rates_kernel=kernel)), oracle_mod.Oracle(desc)
+    rng = np.random.default_rng(4)
+    n = 161
+    st = dict(T=rng.uniform(280, 3000, n), p=10.0 ** rng.uniform(3.5, 7.0, n),
+              Y=np.ascontiguousarray(rng.dirichlet(np.ones(5), size=n).T))
+    ref = parity.run_oracle(om, st)
+    assert np.all(np.isfinite(ref["omega"])) and np.any(ref["omega"] != 0.0)
+    parity.assert_parity(parity.run_gpu(gm, st), ref, f"Troe {which} / {kernel}")
 
 
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
