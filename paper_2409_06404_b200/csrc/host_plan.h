@@ -39,6 +39,12 @@ struct RatesSmemPlanOffsets {
 
 // `opt` is the explicit plan request of crf_mech_create_ex (all zero = automatic); a builder that cannot honour
 // the request returns an empty plan (W = 0) and crf_mech_create_ex reports CRF_EUNSUPPORTED.
+struct RatesGroupPlanOffsets {
+    int W = 0, PPL = 0, maxown = 0, Rc = 0, n_chunks = 0, stage_bytes = 0;
+    size_t chunk = 0, stage = 0, gco = 0, hco = 0, own = 0;
+};
+
 TransportPlanOffsets build_transport_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b);
 RatesPlanOffsets build_rates_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b);
 RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b);
+RatesGroupPlanOffsets build_rates_group_plan(const crf_tables *t, const crf_plan_options &opt, BlockBuilder &b);

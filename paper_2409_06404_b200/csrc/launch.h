@@ -20,11 +20,14 @@ cudaError_t launch_rates_staged(const DevTables &m, const double *T, const doubl
                                 double *omega, double *qdot, cudaStream_t st);
 cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                               double *omega, double *qdot, cudaStream_t st);
+cudaError_t launch_rates_group(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
+                               double *omega, double *qdot, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *inst_per_s);
 // dynamic shared memory per block of the kernel the plan selects (0 for the generic kernels' own sizing): crf_plan_info
 size_t rates_dynamic_smem(const DevTables &m);
 size_t transport_dynamic_smem(const DevTables &m);
 size_t rates_smem_dynamic_smem(const DevTables &m);
+size_t rates_group_dynamic_smem(const DevTables &m);
 size_t rates_staged_dynamic_smem(const DevTables &m);
 size_t transport_tiled_dynamic_smem(const DevTables &m);
 size_t transport_small_dynamic_smem(const DevTables &m);

@@ -157,7 +157,8 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, const crf_plan_o
     Builder B{t, t->Ns, t->Nr, t->N3, t->Nt, t->Nr - t->N3 - t->Nt};
     const int Ns = B.Ns, Nr = B.Nr;
     const int want = opt.rates_kernel;
-    if (Nr == 0 || Ns > 256 || want == CRF_RATES_STAGED || want == CRF_RATES_GENERIC) return o;
+    if (Nr == 0 || Ns > 256 || want == CRF_RATES_STAGED || want == CRF_RATES_GENERIC || want == CRF_RATES_GROUP) return o;
+    if (want == CRF_RATES_AUTO && Ns > 12) return o;  // the warp-group kernel (rates_group.cu)
     for (int r = B.Ne; r < Nr; ++r)
         if (B.generic(r)) return o;  // a third body next to three explicit reactants: staged kernel
     if (!product_form_in_range(B)) return o;

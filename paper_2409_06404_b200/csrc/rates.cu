@@ -149,6 +149,7 @@ cudaError_t launch_b(const DevTables &m, const double *T, const double *p, const
 size_t rates_dynamic_smem(const DevTables &m)
 {
     if (m.rs.W > 0) return rates_smem_dynamic_smem(m);
+    if (m.rg.W > 0) return rates_group_dynamic_smem(m);
     if (m.rp.W > 0) return rates_staged_dynamic_smem(m);
     const size_t per_thread = sizeof(double) * 2 * (size_t)m.Ns;
     return per_thread * (per_thread * 128 <= 100 * 1024 ? 128 : (per_thread * 64 <= 200 * 1024 ? 64 : 32));
@@ -158,6 +159,7 @@ cudaError_t launch_rates(const DevTables &m, const double *T, const double *p, c
                          double *omega, double *qdot, cudaStream_t st)
 {
     if (m.rs.W > 0) return launch_rates_smem(m, T, p, Y, n, omega, qdot, st);
+    if (m.rg.W > 0) return launch_rates_group(m, T, p, Y, n, omega, qdot, st);
     if (m.rp.W > 0) return launch_rates_staged(m, T, p, Y, n, omega, qdot, st);
     const size_t per_thread = sizeof(double) * 2 * (size_t)m.Ns;
     const size_t budget = 100 * 1024;  // two blocks per SM

@@ -1,0 +1,520 @@
+// rates_group.cu -- crf_production_rates, the kernel the library uses whenever the
+// mechanism admits its plan (plan_rates_group.cu); rates_staged.cu (log-space K_c) and rates.cu are the fall-backs.
+//
+// Shape.  W warps share a group of 32 PPL grid points (lane = point, PPL points per lane), so every mechanism
+// coefficient is a warp-uniform shared-memory load.  The kernel is bound by two resources at once, the FP64 pipe and
+// the shared-memory pipe (128 bytes per cycle per SM), so both the FP64 instructions and the shared-memory bytes per
+// reaction are kept as low as the method allows:
+//
+//   activity form   per point and species the block keeps d_k = (p_ref/RT) exp(-g_k/RT) and u_k = C_k / d_k.
+//                   With K_c = prod_products d / prod_reactants d, k_r = k_f / K_c and
+//                   C_k = u_k d_k the rate of progress of step 8 becomes
+//                       q = k_f prod_reactants d_a (prod_reactants u_a - prod_products u_b) [M]
+//                   one exponential (k_f) per reaction, no division, and the product side needs u only: 96 bytes of
+//                   state per reaction and two points instead of 128.  crf_mech_create admits this form only if every
+//                   factor stays a normal double for 250 K <= T <= 5000 K (plan_rates_group.cu).
+//   pair layout     the PPL = 2 points of a lane are adjacent in every row (state rows U_k, D_k, q rows): one 128-bit
+//                   access serves both.
+//   reaction stage  the reactions are cut into a few chunks; a chunk's reactions are dealt to the warps balanced by
+//                   cost (a falloff reaction costs six elementary ones), q_r -> q buffer.
+//   species stage   every species is owned by one warp (balanced by incidence count); the owner sums nu_kr q_r over the
+//                   chunk's incidence list of the species (4-byte entries: q row | sign) into register accumulators
+//                   that live for the whole kernel: omega never touches shared memory.
+//   staging         a chunk's tables (records, Troe sets, third-body lists, incidence lists) are one contiguous block,
+//                   copied global -> shared by ONE bulk copy (cp.async.bulk, completion on an mbarrier) issued by one
+//                   thread while the previous chunk is evaluated.
+// Troe falloff is evaluated in base 2 (log2 F = log2 F_cent / (1 + f1^2)) with a branch-free logarithm.
+// Accuracy: 2^y by a degree-8 polynomial (relative error 1.1e-12), sized to the tolerance of omega and qdot
+// (1e-10 of the gross rate, BASELINE.json north_star), not to 1 ulp.
+#include "crf_internal.h"
+#include "fastmath.cuh"
+#include "launch.h"
+
+namespace {
+
+// 2^f on [-1/2, 1/2], degree 8 (Chebyshev-node interpolant, relative error 1.06e-12), and the odd atanh series, in
+// constant memory: the FP64 instructions take the coefficients as constant-bank operands
+__constant__ double kExp2[9] = {0x1.0000000000000p+0,  0x1.62e42fef84cf0p-1,  0x1.ebfbdff823cedp-3,
+                                0x1.c6b08dd6fd234p-5,  0x1.3b2ab7181b755p-7,  0x1.5d8745a728441p-10,
+                                0x1.4308ac85aa947p-13, 0x1.00dc4a532fb8ep-16, 0x1.63d136366db24p-20};
+__constant__ double kAtanh[7] = {1.0, 1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0};
+
+// 2^y; the exponent is clamped from below: an underflowing rate constant becomes a negligible number instead of
+// wrapping into the sign bit.  |y| < 2^31 (callers clamp arguments that can be arbitrarily large).
+__device__ __forceinline__ double exp2r(double y)
+{
+    const double magic = 6755399441055744.0;  // 1.5 * 2^52
+    const double t = __dadd_rn(y, magic);
+    const int k = max(__double2loint(t), -1000);
+    const double f = __dsub_rn(y, __dsub_rn(t, magic));
+    double p = kExp2[8];
+#pragma unroll
+    for (int i = 7; i >= 0; --i) p = fma(p, f, kExp2[i]);
+    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+// 1/x for normal x: MUFU.RCP64H seed (relative error < 2^-20) and one cubic Newton step
+__device__ __forceinline__ double rcp_fast(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    return fma(y, fma(e, e, e), y);
+}
+
+// log2(x) for normal x > 0, branch-free: x = 2^e m, m in [sqrt(1/2), sqrt(2)), ln m = 2 atanh((m-1)/(m+1));
+// series truncated after s^13 (|s| <= 0.172: absolute error 2e-12)
+__device__ __forceinline__ double log2_fast(double x)
+{
+    int hi = __double2hiint(x);
+    const int e = (hi - 0x3fe6a09e) >> 20;
+    hi -= e << 20;
+    const double m = __hiloint2double(hi, __double2loint(x));
+    const double s = (m - 1.0) * rcp_fast(m + 1.0);
+    const double z = s * s;
+    double p = kAtanh[6];
+#pragma unroll
+    for (int i = 5; i >= 0; --i) p = fma(p, z, kAtanh[i]);
+    return fma(s * (2.0 * crf::kLog2e), p, (double)e);
+}
+
+// ---- rows: [lane][PPL] doubles; a lane's PPL points are adjacent -------------------------------------------------
+template <int PPL>
+__device__ __forceinline__ void ld_row(const char *p, double (&v)[PPL])
+{
+    if (PPL == 2) {
+        const double2 t = *reinterpret_cast<const double2 *>(p);
+        v[0] = t.x, v[PPL - 1] = t.y;
+    } else {
+        v[0] = *reinterpret_cast<const double *>(p);
+    }
+}
+template <int PPL>
+__device__ __forceinline__ void st_row(char *p, const double (&v)[PPL])
+{
+    if (PPL == 2)
+        *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[PPL - 1]);
+    else
+        *reinterpret_cast<double *>(p) = v[0];
+}
+__device__ __forceinline__ uint4 ldsu4(const char *p) { return *reinterpret_cast<const uint4 *>(p); }
+__device__ __forceinline__ uint2 ldsu2(const char *p) { return *reinterpret_cast<const uint2 *>(p); }
+__device__ __forceinline__ double2 lds2(const char *p) { return *reinterpret_cast<const double2 *>(p); }
+
+// global rows: the PPL points of a lane are adjacent: i0, i0 + 1 (one 128-bit access per row when n is even)
+template <int PPL>
+__device__ __forceinline__ void load_row(const double *__restrict__ row, int64_t i0, int64_t n, bool vec, double (&v)[PPL])
+{
+    if (PPL == 2 && vec && i0 + 1 < n) {
+        const double2 t = *reinterpret_cast<const double2 *>(row + i0);
+        v[0] = t.x, v[PPL - 1] = t.y;
+    } else {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) v[u] = row[min(i0 + u, n - 1)];
+    }
+}
+template <int PPL>
+__device__ __forceinline__ void store_row(double *__restrict__ row, int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
+{
+    if (PPL == 2 && vec && i0 + 1 < n) {
+        *reinterpret_cast<double2 *>(row + i0) = make_double2(v[0], v[PPL - 1]);
+    } else {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u)
+            if (i0 + u < n) row[i0 + u] = v[u];
+    }
+}
+
+// ---- bulk copy global -> shared with mbarrier completion (TMA, non-tensor form) ------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+template <int PPL>
+struct Ctx {
+    double T[PPL], L[PPL], rT[PPL];  // T, ln T, 1/T
+    double Csum[PPL];                // p/(R T)
+};
+
+// q of one reaction at the PPL points of this lane.  rec: the 48-byte record; tr: its Troe set (kind 2); blk: the chunk
+// block (third-body lists); sl: the state at this lane (row offsets come from the record; D_k is RB bytes behind U_k).
+template <int KIND, bool GENERIC, int PPL>
+__device__ __forceinline__ void reaction_q(const char *blk, const char *rec, const char *tr, const char *sl,
+                                           const Ctx<PPL> &c, double (&q)[PPL])
+{
+    constexpr int RB = 256 * PPL;
+    const double2 A = lds2(rec);        // log2e lnA, log2e beta
+    const double2 Ex = lds2(rec + 16);  // -log2e Ea/R, (x0, x1)
+    const uint4 S = ldsu4(rec + 32);    // a0, a1, b0, b1
+    const unsigned x0 = (unsigned)__double2loint(Ex.y), x1 = (unsigned)__double2hiint(Ex.y);
+    double ua0[PPL], ua1[PPL], da0[PPL], da1[PPL], ub0[PPL], ub1[PPL];
+    ld_row<PPL>(sl + S.x, ua0), ld_row<PPL>(sl + S.x + RB, da0);
+    ld_row<PPL>(sl + S.y, ua1), ld_row<PPL>(sl + S.y + RB, da1);
+    ld_row<PPL>(sl + S.z, ub0), ld_row<PPL>(sl + S.w, ub1);
+    double M[PPL];
+    if (KIND != 0) {
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) M[u] = c.Csum[u];
+        const char *e = blk + x0, *e1 = e + 16 * x1;
+        for (; e < e1; e += 16) {
+            const uint4 en = ldsu4(e);
+            const double coef = __hiloint2double((int)en.y, (int)en.x);
+            double uu[PPL], dd[PPL];
+            ld_row<PPL>(sl + en.z, uu), ld_row<PPL>(sl + en.z + RB, dd);
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) M[u] = fma(coef, uu[u] * dd[u], M[u]);  // C_k = u_k d_k
+        }
+    }
+    double ua2[PPL], da2[PPL], ub2[PPL];
+    if (GENERIC) ld_row<PPL>(sl + x0, ua2), ld_row<PPL>(sl + x0 + RB, da2), ld_row<PPL>(sl + x1, ub2);
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) {
+        const double yinf = fma(A.y, c.L[u], fma(Ex.x, c.rT[u], A.x));  // log2 k_f (high-pressure limit)
+        double dd = da0[u] * da1[u], pb = ub0[u] * ub1[u], net;
+        if (GENERIC) {
+            dd *= da2[u], pb *= ub2[u];
+            net = fma(ua0[u] * ua1[u], ua2[u], -pb);
+        } else {
+            net = fma(ua0[u], ua1[u], -pb);
+        }
+        if (KIND == 0) q[u] = (exp2r(yinf) * dd) * net;
+        if (KIND == 1) q[u] = (exp2r(yinf) * dd) * (M[u] * net);
+        if (KIND == 2) {
+            // Troe falloff in base 2
+            const double2 t01 = lds2(tr), t23 = lds2(tr + 16), t45 = lds2(tr + 32), t67 = lds2(tr + 48);
+            const double y0 = fma(t01.y, c.L[u], fma(t23.x, c.rT[u], t01.x));
+            const double l2Pr = (y0 - yinf) + log2_fast(fmax(M[u], 1.0e-300));  // log2(k_0 [M] / k_inf)
+            const double al = t23.y;
+            // (the arguments are clamped BEFORE the range reduction: Chemkin-style switched-off terms, T3 = 1e-30 or
+            // T2 = 1e30 / inf, give arguments of -1e33 or -inf, whose integer part has no meaning as an exponent)
+            const double Fc = fma(1.0 - al, exp2r(fmax(c.T[u] * t45.x, -1022.0)),
+                                  fma(al, exp2r(fmax(c.T[u] * t45.y, -1022.0)), exp2r(fmax(t67.x * c.rT[u], -1022.0))));
+            const double l2Fc = log2_fast(fmax(Fc, 1.0e-300));
+            const double l10_2 = 0.30102999566398119521;
+            const double lFc = l10_2 * l2Fc;
+            const double x = fma(l10_2, l2Pr, fma(-0.67, lFc, -0.4));  // log10 P_r + c
+            const double f1 = x * rcp_fast(fma(-0.14, x, fma(-1.27, lFc, 0.75)));
+            const double l2F = l2Fc * rcp_fast(fma(f1, f1, 1.0));
+            const double Pred = exp2r(l2Pr);
+            q[u] = (exp2r(yinf + l2F) * dd) * ((Pred * rcp_fast(1.0 + Pred)) * net);
+        }
+    }
+}
+
+template <int KIND, bool GENERIC, int PPL>
+__device__ __forceinline__ void reaction_loop(const char *blk, const char *&rec, const char *&tr, char *&qp, int count,
+                                              const char *sl, const Ctx<PPL> &c)
+{
+    constexpr int RB = 256 * PPL;
+#pragma unroll 1
+    for (int i = 0; i < count; ++i) {
+        double q[PPL];
+        reaction_q<KIND, GENERIC, PPL>(blk, rec, tr, sl, c, q);
+        st_row<PPL>(qp, q);
+        rec += 48, qp += RB;
+        if (KIND == 2) tr += 64;
+    }
+}
+
+// one incidence entry: om += (+-1) q[row]
+template <int PPL>
+__device__ __forceinline__ void gather(unsigned en, const char *sQl, double (&om)[PPL])
+{
+    double q[PPL];
+    ld_row<PPL>(sQl + (en & 0x7fffffffu), q);
+    const double nu = __hiloint2double((int)((en & 0x80000000u) | 0x3ff00000u), 0);
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) om[u] = fma(nu, q[u], om[u]);
+}
+
+template <int W, int PPL, int MAXOWN>
+__global__ void __launch_bounds__(32 * W, 16 / W)
+    rates_group_kernel(DevTables m, const double *__restrict__ T, const double *__restrict__ p,
+                       const double *__restrict__ Y, int64_t n, double *__restrict__ omega, double *__restrict__ qdot)
+{
+    extern __shared__ double2 sm2[];
+    __shared__ uint64_t mbar[2];
+    __shared__ int4 sChunk[64];
+    const RatesGroupPlan &rg = m.rg;
+    constexpr int RB = 256 * PPL, LB = 8 * PPL;
+    const int Ns = m.Ns;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    char *sS = reinterpret_cast<char *>(sm2);                 // [Ns + 1][2][RB] (U_k, D_k); row Ns = (1, 1)
+    char *sQ = sS + (size_t)(Ns + 1) * 2 * RB;                // [max(Rc, W)][RB] q_r; also the reduction scratch
+    char *sStage = sQ + (size_t)max(rg.Rc, W) * RB;           // [2][stage_bytes]
+    char *sl = sS + lane * LB;
+    char *sQl = sQ + lane * LB;
+    const int sb = rg.stage_bytes, nch = rg.n_chunks;
+
+    if (threadIdx.x == 0) {
+        mbar_init(&mbar[0], 1);
+        mbar_init(&mbar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int ci = threadIdx.x; ci < nch && ci < 64; ci += 32 * W) sChunk[ci] = __ldg(rg.chunk + ci);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        // chunk 0 -> buffer 0; buffer 1 is free until chunk 1 is prefetched: it carries the g/(RT) sets for the prologue
+        bulk_load(sStage, rg.stage + sChunk[0].x, (unsigned)sChunk[0].y, &mbar[0]);
+        bulk_load(sStage + sb, rg.gco, 128u * Ns, &mbar[1]);
+    }
+
+    const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * PPL;
+    const bool vec = (n & 1) == 0;
+    Ctx<PPL> c;
+    double pi[PPL];
+    load_row<PPL>(T, i0, n, vec, c.T);
+    load_row<PPL>(p, i0, n, vec, pi);
+    // ---- a1: Z_k = Y_k / W_k; warp w takes species w, w + W, ...: all row loads of the warp are in flight together
+    double z[MAXOWN][PPL];
+#pragma unroll
+    for (int s = 0; s < MAXOWN; ++s) {
+        const int k = warp + W * s;
+        if (k < Ns) load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, z[s]);
+    }
+    double lc02[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) {
+        c.L[u] = log(c.T[u]);
+        c.rT[u] = 1.0 / c.T[u];
+        lc02[u] = crf::kLog2e * (log(m.p_ref / CRF_R_GAS) - c.L[u]);  // log2(p_ref/(R T))
+        c.Csum[u] = pi[u] * c.rT[u] * (1.0 / CRF_R_GAS);
+    }
+    mbar_wait(&mbar[1], 0);
+    const double2 *sG = reinterpret_cast<const double2 *>(sStage + sb);
+    double invW[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) invW[u] = 0.0;
+#pragma unroll
+    for (int s = 0; s < MAXOWN; ++s) {
+        const int k = warp + W * s;
+        if (k < Ns) {
+            const double rW = sG[8 * k + 7].y;
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) {
+                z[s][u] *= rW;
+                invW[u] += z[s][u];
+            }
+        }
+    }
+    double *sred = reinterpret_cast<double *>(sQ);  // [W][PPL][32], valid outside the chunk loop
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) sred[(warp * PPL + u) * 32 + lane] = invW[u];
+    __syncthreads();
+    double rho[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
+        rho[u] = pi[u] / (CRF_R_GAS * c.T[u] * s);
+    }
+    // ---- a2: d_k = 2^(log2(p_ref/RT) - log2e g_k/RT), u_k = rho Z_k / d_k
+#pragma unroll
+    for (int s = 0; s < MAXOWN; ++s) {
+        const int k = warp + W * s;
+        if (k >= Ns) continue;
+        const double2 *g = sG + 8 * k;
+        const double2 l01 = g[0], l23 = g[1], l45 = g[2], l6t = g[3];
+        const double2 h01 = g[4], h23 = g[5], h45 = g[6], h6w = g[7];
+        double uu[PPL], dd[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) {
+            const double Tu = c.T[u], oml = 1.0 - c.L[u];
+            double lo = fma(Tu, l45.x, l23.y);
+            lo = fma(Tu, lo, l23.x);
+            lo = fma(Tu, lo, l01.y);
+            lo = fma(Tu, lo, l6t.x);
+            lo = fma(l45.y, c.rT[u], lo);
+            lo = fma(l01.x, oml, lo);
+            double hi = fma(Tu, h45.x, h23.y);
+            hi = fma(Tu, hi, h23.x);
+            hi = fma(Tu, hi, h01.y);
+            hi = fma(Tu, hi, h6w.x);
+            hi = fma(h45.y, c.rT[u], hi);
+            hi = fma(h01.x, oml, hi);
+            const double g2 = Tu <= l6t.y ? lo : hi;
+            dd[u] = exp2r(lc02[u] - g2);
+            uu[u] = (rho[u] * z[s][u]) * rcp_fast(dd[u]);
+        }
+        st_row<PPL>(sl + (size_t)k * 2 * RB, uu);
+        st_row<PPL>(sl + (size_t)k * 2 * RB + RB, dd);
+    }
+    if (warp == 0) {
+        double one[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) one[u] = 1.0;
+        st_row<PPL>(sl + (size_t)Ns * 2 * RB, one);
+        st_row<PPL>(sl + (size_t)Ns * 2 * RB + RB, one);
+    }
+    __syncthreads();  // the state is complete; everyone is done with the g sets and the reduction scratch
+
+    double om[MAXOWN][PPL];
+#pragma unroll
+    for (int s = 0; s < MAXOWN; ++s)
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) om[s][u] = 0.0;
+
+    for (int ci = 0; ci < nch; ++ci) {
+        const char *blk = sStage + (size_t)(ci & 1) * sb;
+        if (threadIdx.x == 0) {
+            char *dst = sStage + (size_t)((ci + 1) & 1) * sb;
+            if (ci + 1 < nch)
+                bulk_load(dst, rg.stage + sChunk[ci + 1].x, (unsigned)sChunk[ci + 1].y, &mbar[(ci + 1) & 1]);
+            else  // behind the last chunk: the h/(RT) sets for the epilogue
+                bulk_load(dst, rg.hco, 128u * Ns, &mbar[(ci + 1) & 1]);
+        }
+        mbar_wait(&mbar[ci & 1], (unsigned)((ci >> 1) + (ci & 1)) & 1u);
+        {
+            const uint4 hw = ldsu4(blk + 32 * warp);  // records, first q row, slot table, Troe sets
+            const uint2 cn = ldsu2(blk + 32 * warp + 16);
+            const char *rec = blk + hw.x, *tr = blk + hw.w;
+            char *qp = sQl + hw.y;
+            reaction_loop<0, false, PPL>(blk, rec, tr, qp, (int)(cn.x & 0xffffu), sl, c);
+            if (cn.x >> 16) reaction_loop<0, true, PPL>(blk, rec, tr, qp, (int)(cn.x >> 16), sl, c);
+            if (cn.y & 0xffffu) reaction_loop<1, false, PPL>(blk, rec, tr, qp, (int)(cn.y & 0xffffu), sl, c);
+            if (cn.y >> 16) reaction_loop<2, false, PPL>(blk, rec, tr, qp, (int)(cn.y >> 16), sl, c);
+            __syncthreads();
+            // ---- species stage: the warp's entries are contiguous (slot-major); slot s ends at end[s]
+            const char *tab = blk + hw.z;
+            unsigned e = *reinterpret_cast<const unsigned *>(tab + 4 * MAXOWN);
+#pragma unroll
+            for (int s4 = 0; s4 < MAXOWN; s4 += 4) {
+                const uint4 ends = ldsu4(tab + 4 * s4);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int s = s4 + j;
+                    const unsigned end = j == 0 ? ends.x : (j == 1 ? ends.y : (j == 2 ? ends.z : ends.w));
+#pragma unroll 1
+                    for (; e + 8 <= end; e += 8) {
+                        const uint2 en = ldsu2(blk + e);
+                        gather<PPL>(en.x, sQl, om[s]);
+                        gather<PPL>(en.y, sQl, om[s]);
+                    }
+                    if (e < end) gather<PPL>(*reinterpret_cast<const unsigned *>(blk + e), sQl, om[s]);
+                    e = (end + 7u) & ~7u;
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- store omega; a9: qdot = -sum_k h_k omega_k
+    mbar_wait(&mbar[nch & 1], (unsigned)((nch >> 1) + (nch & 1)) & 1u);
+    const double2 *sH = reinterpret_cast<const double2 *>(sStage + (size_t)(nch & 1) * sb);
+    double qd[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) qd[u] = 0.0;
+#pragma unroll
+    for (int s = 0; s < MAXOWN; ++s) {
+        const int k = __ldg(rg.own + warp * MAXOWN + s);
+        if (k >= 0) {
+            const double2 *h = sH + 8 * k;
+            const double2 l01 = h[0], l23 = h[1], l45 = h[2], l6t = h[3];
+            const double2 h01 = h[4], h23 = h[5], h45 = h[6];
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) {
+                const double Tu = c.T[u];
+                double lo = fma(Tu, l45.x, l23.y);
+                lo = fma(Tu, lo, l23.x);
+                lo = fma(Tu, lo, l01.y);
+                lo = fma(Tu, lo, l01.x);
+                lo = fma(l45.y, c.rT[u], lo);
+                double hi = fma(Tu, h45.x, h23.y);
+                hi = fma(Tu, hi, h23.x);
+                hi = fma(Tu, hi, h01.y);
+                hi = fma(Tu, hi, h01.x);
+                hi = fma(h45.y, c.rT[u], hi);
+                qd[u] = fma(-(Tu <= l6t.y ? lo : hi), om[s][u], qd[u]);
+            }
+            store_row<PPL>(omega + (int64_t)k * n, i0, n, vec, om[s]);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) sred[(warp * PPL + u) * 32 + lane] = qd[u];
+    __syncthreads();
+    if (warp == 0) {
+        double out[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) {
+            double s = 0.0;
+#pragma unroll
+            for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
+            out[u] = s * (CRF_R_GAS * c.T[u]);
+        }
+        store_row<PPL>(qdot, i0, n, vec, out);
+    }
+}
+
+template <int W, int PPL, int MAXOWN>
+cudaError_t launch_k(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
+                     double *qdot, cudaStream_t st)
+{
+    const size_t smem = rates_group_dynamic_smem(m);
+    cudaError_t e = cudaFuncSetAttribute(rates_group_kernel<W, PPL, MAXOWN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem);
+    if (e != cudaSuccess) return e;
+    const int64_t per_block = 32 * PPL;
+    rates_group_kernel<W, PPL, MAXOWN><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, p, Y, n,
+                                                                                                         omega, qdot);
+    crf_count_launch();
+    return cudaGetLastError();
+}
+
+template <int W, int PPL>
+cudaError_t launch_wp(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
+                      double *qdot, cudaStream_t st)
+{
+    switch (m.rg.maxown) {
+    case 4: return launch_k<W, PPL, 4>(m, T, p, Y, n, omega, qdot, st);
+    case 8: return launch_k<W, PPL, 8>(m, T, p, Y, n, omega, qdot, st);
+    case 16: return launch_k<W, PPL, 16>(m, T, p, Y, n, omega, qdot, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
+
+size_t rates_group_dynamic_smem(const DevTables &m)
+{
+    const RatesGroupPlan &rg = m.rg;
+    const size_t rb = 256 * (size_t)rg.PPL;
+    return (size_t)(m.Ns + 1) * 2 * rb + (size_t)(rg.Rc > rg.W ? rg.Rc : rg.W) * rb + 2 * (size_t)rg.stage_bytes;
+}
+
+cudaError_t launch_rates_group(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
+                               double *omega, double *qdot, cudaStream_t st)
+{
+    switch (m.rg.W * 10 + m.rg.PPL) {
+    case 41: return launch_wp<4, 1>(m, T, p, Y, n, omega, qdot, st);
+    case 42: return launch_wp<4, 2>(m, T, p, Y, n, omega, qdot, st);
+    case 81: return launch_wp<8, 1>(m, T, p, Y, n, omega, qdot, st);
+    case 82: return launch_wp<8, 2>(m, T, p, Y, n, omega, qdot, st);
+    case 161: return launch_wp<16, 1>(m, T, p, Y, n, omega, qdot, st);
+    case 162: return launch_wp<16, 2>(m, T, p, Y, n, omega, qdot, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
