@@ -20,7 +20,7 @@ extern "C" {
 #define CRF_RATES_AUTO 0
 #define CRF_RATES_GENERIC 1 /* one thread per point, libm exponentials, any mechanism (rates.cu) */
 #define CRF_RATES_STAGED 2  /* warp groups, log-space K_c: two exponentials per reaction (rates_staged.cu) */
-#define CRF_RATES_GROUP 3   /* warp groups, product form of K_c, chunk tables in shared memory (rates_smem.cu) */
+#define CRF_RATES_GROUP 3   /* warp groups, activity form of K_c, u rows in tensor memory, chunk tables staged by bulk copies (rates_group.cu) */
 #define CRF_RATES_THREAD 4  /* one thread per point, product form of K_c, small mechanisms (rates_smem.cu) */
 
 #define CRF_TRANSPORT_AUTO 0
@@ -41,7 +41,8 @@ typedef struct crf_plan_options {
     int32_t transport_W;      /* warps sharing a point group: 1, 2, 4 or 8 (TILED) */
     int32_t transport_PPL;    /* points per lane: 1 or 2 (TILED) */
     int32_t transport_panel;  /* column blocks per Wilke panel (TILED) */
-    int32_t reserved[8];      /* must be 0 */
+    int32_t rates_tmem;       /* GROUP: 0 = u rows in tensor memory when they fit, 1 = in shared memory, 2 = require tensor memory */
+    int32_t reserved[7];      /* must be 0 */
 } crf_plan_options;
 
 /* What a mechanism will run. */
@@ -51,7 +52,8 @@ typedef struct crf_plan_info {
     int32_t transport_kernel; /* CRF_TRANSPORT_* (never AUTO) */
     int32_t transport_W, transport_PPL, transport_nb, transport_stage_blocks, transport_stage_bytes,
         transport_smem_bytes;
-    int32_t reserved[8];
+    int32_t rates_tmem_cols; /* tensor-memory columns a block of the GROUP kernel allocates (0: u rows in shared memory) */
+    int32_t reserved[7];
 } crf_plan_info;
 
 /* crf_mech_create with an explicit plan request (options may be NULL = all automatic). */

@@ -167,14 +167,14 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
     const RatesGroupPlanOffsets rgo = rso.W > 0 ? RatesGroupPlanOffsets() : build_rates_group_plan(t, opt, b);
     // what will run, and whether that is what was asked for
     crf_plan_info info{};
-    info.rates_kernel = rso.W > 0 ? (rso.PPL == 4 ? CRF_RATES_THREAD : 5)
+    info.rates_kernel = rso.W > 0 ? CRF_RATES_THREAD
                                   : (rgo.W > 0 ? CRF_RATES_GROUP : (rpo.W > 0 ? CRF_RATES_STAGED : CRF_RATES_GENERIC));
     if (rso.W > 0)
         info.rates_W = rso.W, info.rates_PPL = rso.PPL, info.rates_Rc = rso.Rc, info.rates_chunks = rso.n_chunks,
         info.rates_stage_bytes = rso.stage_bytes;
     else if (rgo.W > 0)
         info.rates_W = rgo.W, info.rates_PPL = rgo.PPL, info.rates_Rc = rgo.Rc, info.rates_chunks = rgo.n_chunks,
-        info.rates_stage_bytes = rgo.stage_bytes;
+        info.rates_stage_bytes = rgo.stage_bytes, info.rates_tmem_cols = rgo.tm_cols;
     else if (rpo.W > 0)
         info.rates_W = rpo.W, info.rates_PPL = 1, info.rates_Rc = rpo.Rc, info.rates_chunks = rpo.n_chunks;
     info.transport_kernel = tpo.W > 0 ? CRF_TRANSPORT_TILED : (tpo.small_n > 0 ? CRF_TRANSPORT_SMALL : CRF_TRANSPORT_GENERIC);
@@ -233,7 +233,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
     rs.gco = D(rso.gco), rs.hco = D(rso.hco);
     RatesGroupPlan &rg = d.rg;
     rg.W = rgo.W, rg.PPL = rgo.PPL, rg.maxown = rgo.maxown, rg.Rc = rgo.Rc, rg.n_chunks = rgo.n_chunks,
-    rg.stage_bytes = rgo.stage_bytes;
+    rg.stage_bytes = rgo.stage_bytes, rg.q_rows = rgo.q_rows, rg.tm_cols = rgo.tm_cols, rg.log2_c0 = rgo.log2_c0;
     rg.chunk = reinterpret_cast<const int4 *>(base + rgo.chunk);
     rg.stage = base + rgo.stage;
     rg.gco = D(rgo.gco), rg.hco = D(rgo.hco);

@@ -81,28 +81,34 @@ struct RatesSmemPlan {
 
 // Plan of the warp-group crf_production_rates kernel (rates_group.cu).  W warps share 32 PPL points.  The reactions are
 // cut into n_chunks chunks of at most Rc reactions; a chunk's reactions are dealt to the W warps (balanced by cost), its
-// q_r go to a shared q buffer of Rc + 1 rows (row Rc stays zero), and each warp then sums nu_kr q_r for the species it
-// owns.  Everything a chunk needs is one contiguous block of `stage`, copied into shared memory by one bulk copy
-// (cp.async.bulk + mbarrier) while the previous chunk is evaluated.  Block layout (byte offsets from its start):
+// q_r go to a shared q buffer (row Rc stays zero), and each warp then sums q_r for the species it owns.  Everything a
+// chunk needs is one contiguous block of `stage`, copied into shared memory by one bulk copy (cp.async.bulk + mbarrier)
+// while the previous chunk is evaluated.  Block layout (byte offsets from its start):
 //   [0, 32 W)      per warp: u32 records, u32 first q row (byte offset in the q buffer), u32 slot table, u32 Troe sets,
 //                  u16 n[4] = reactions of kind elementary / elementary with three slots / third body / falloff
-//   records        48 bytes per reaction, in the warp's processing order (the four kinds in that order; q rows are
-//                  consecutive): f64 log2(e) lnA, f64 log2(e) beta, f64 -log2(e) Ea/R, u32 x0, u32 x1, u32 a0, a1, b0, b1
-//                  (byte offsets of the reactant / product species in the state; x0, x1 = third reactant / product, or
-//                  offset / count of the third-body list); empty slots point at the dummy species, row Ns
+//   records        64 bytes per reaction, in the warp's processing order (the four kinds in that order; q rows are
+//                  consecutive): f64 log2(e) lnA, f64 log2(e) beta, f64 -log2(e) Ea/R, u32 b0u, b1u, u32 a0d, a1d, a0u,
+//                  a1u, u32 x0, x1, x0u, x1u.  *d = byte offset of the species' d row in the shared-memory state, *u =
+//                  handle of its u row (tensor-memory column, or byte offset of the row in shared memory); a = reactants,
+//                  b = products, x0/x0u = third reactant, x1u = third product (kind "three slots"), or x0/x1 = offset /
+//                  count of the third-body list; empty slots point at the dummy species, row Ns
 //   Troe sets      64 bytes per falloff reaction of the warp, in order
-//   third-body     entries {f64 efficiency - 1, u32 state offset, u32 0}
-//   slot table     per warp: u32 end[maxown] of the incidence list of each owned slot, u32 start of the first list
-//   entries        u32 = byte offset of the q row | sign << 31 (a coefficient of +-2 is two entries); a slot's list
-//                  starts 8-byte aligned
-// State: species k owns two rows of 256 PPL bytes at 512 PPL k: U (u_k = C_k / d_k) then D (d_k), [lane][PPL].
+//   third-body     entries {f64 efficiency - 1, u32 d offset, u32 u handle}
+//   slot table     per warp: u32 {end of the plus list, end of the minus list}[maxown], u32 start of the first list
+//   entries        u32 = byte offset of the q row (a coefficient of +-2 is two entries); a list starts 8-byte aligned
+//                  and has even length (padded with the zero row Rc)
+// State: d_k = (p_ref/RT) exp(-g_k/RT) and u_k = C_k / d_k, rows of 256 PPL bytes [lane][PPL].  Shared memory: d rows
+// [Ns + 1], then (tm_cols = 0) u rows [Ns + 1].  tm_cols > 0: u_k lives in tensor memory, columns [2 PPL k, 2 PPL (k + 1)).
 struct RatesGroupPlan {
     int W;            // warps sharing a point group; 0 = no plan
     int PPL;          // points per lane (1 or 2)
     int maxown;       // owned-species slots per warp (4, 8 or 16)
-    int Rc;           // q buffer rows (largest chunk)
+    int Rc;           // largest chunk; q buffer row Rc is the zero row
+    int q_rows;       // rows of the q buffer (>= Rc + 1; the prologue's scratch too)
+    int tm_cols;      // tensor-memory columns a block allocates (power of two), 0 = U in shared memory
     int n_chunks;
     int stage_bytes;  // largest chunk block, multiple of 16
+    double log2_c0;   // log2(p_ref / R)
     const int4 *chunk;           // [n_chunks]: x = byte offset of the block in stage, y = block bytes, z = reactions
     const unsigned char *stage;
     const double *gco;  // [Ns][16]: log2(e) g/(RT) Horner sets, low range 0-6, high range 8-14, 7 = Tmid, 15 = 1/W

@@ -40,7 +40,8 @@ struct RatesSmemPlanOffsets {
 // `opt` is the explicit plan request of crf_mech_create_ex (all zero = automatic); a builder that cannot honour
 // the request returns an empty plan (W = 0) and crf_mech_create_ex reports CRF_EUNSUPPORTED.
 struct RatesGroupPlanOffsets {
-    int W = 0, PPL = 0, maxown = 0, Rc = 0, n_chunks = 0, stage_bytes = 0;
+    int W = 0, PPL = 0, maxown = 0, Rc = 0, q_rows = 0, tm_cols = 0, n_chunks = 0, stage_bytes = 0;
+    double log2_c0 = 0.0;
     size_t chunk = 0, stage = 0, gco = 0, hco = 0, own = 0;
 };
 

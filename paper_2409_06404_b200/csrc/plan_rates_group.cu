@@ -28,8 +28,8 @@ struct Mech {
     // relative cost of one reaction in the reaction stage (FP64 + shared-memory work; an elementary reaction = 1)
     double cost(int r) const
     {
-        const double base = kind(r) == 2 ? 6.5 : (kind(r) == 1 ? 1.15 : 1.0);
-        return base + (generic(r) ? 0.25 : 0.0) + 0.12 * n_eff(r);
+        const double base = kind(r) == 2 ? 7.0 : (kind(r) == 1 ? 1.15 : 1.0);
+        return base + (generic(r) ? 0.25 : 0.0) + 0.22 * n_eff(r);
     }
 };
 
@@ -143,13 +143,18 @@ std::vector<int> deal_species(const Mech &B, int W, int maxown)
 
 // One chunk block (layout: RatesGroupPlan in crf_internal.h)
 std::vector<unsigned char> chunk_block(const Mech &B, const Chunk &ch, const std::vector<int> &own, int PPL, int W,
-                                       int maxown, int Rc)
+                                       int maxown, int Rc, bool tm)
 {
     const crf_tables *t = B.t;
     const int Ns = B.Ns;
-    const unsigned rowb = 256u * PPL;   // bytes of one row (32 lanes x PPL doubles)
-    const unsigned srow = 2u * rowb;    // a species owns two rows of the state: U then D
-    auto row_of = [&](int k) { return (unsigned)(k >= 0 ? k : Ns) * srow; };  // row Ns: the dummy species
+    const unsigned rowb = 256u * PPL;  // bytes of one row (32 lanes x PPL doubles)
+    // d row k: byte offset k rowb in the shared-memory state; u row k: tensor-memory column 2 PPL k, or the shared-memory
+    // row Ns + 1 + k; empty slots point at the dummy species, row Ns (u = d = 1)
+    auto d_of = [&](int k) { return (unsigned)(k >= 0 ? k : Ns) * rowb; };
+    auto u_of = [&](int k) {
+        const unsigned kk = (unsigned)(k >= 0 ? k : Ns);
+        return tm ? 2u * PPL * kk : (unsigned)(Ns + 1 + kk) * rowb;
+    };
     const size_t hdr = 32 * (size_t)W;
     std::vector<unsigned char> v(hdr, 0);
     auto align16 = [&]() { v.resize((v.size() + 15) & ~size_t(15), 0); };
@@ -163,7 +168,7 @@ std::vector<unsigned char> chunk_block(const Mech &B, const Chunk &ch, const std
         const WarpList &wl = ch.warps[w];
         align16();
         const size_t rec0 = v.size();
-        v.resize(rec0 + 48 * wl.rx.size(), 0);
+        v.resize(rec0 + 64 * wl.rx.size(), 0);
         uint16_t cnt[4] = {0, 0, 0, 0};
         size_t troe0 = 0;
         int n_troe = 0;
@@ -176,11 +181,17 @@ std::vector<unsigned char> chunk_block(const Mech &B, const Chunk &ch, const std
         for (size_t i = 0; i < wl.rx.size(); ++i) {
             const int r = wl.rx[i];
             ++cnt[B.kind(r) == 0 ? (B.generic(r) ? 1 : 0) : B.kind(r) + 1];
-            const size_t o = rec0 + 48 * i;
+            const size_t o = rec0 + 64 * i;
             put(v, o + 0, crf::kLog2e * t->lnA[r]);
             put(v, o + 8, crf::kLog2e * t->beta[r]);
             put(v, o + 16, -crf::kLog2e * t->Ea_R[r]);
-            unsigned x0 = row_of(B.slot(t->reac, 2, r)), x1 = row_of(B.slot(t->prod, 2, r));
+            put(v, o + 24, u_of(B.slot(t->prod, 0, r)));
+            put(v, o + 28, u_of(B.slot(t->prod, 1, r)));
+            put(v, o + 32, d_of(B.slot(t->reac, 0, r)));
+            put(v, o + 36, d_of(B.slot(t->reac, 1, r)));
+            put(v, o + 40, u_of(B.slot(t->reac, 0, r)));
+            put(v, o + 44, u_of(B.slot(t->reac, 1, r)));
+            unsigned x0 = d_of(B.slot(t->reac, 2, r)), x1 = 0;
             if (B.kind(r) != 0) {
                 const int mrow = r - B.Ne;
                 align16();
@@ -190,15 +201,14 @@ std::vector<unsigned char> chunk_block(const Mech &B, const Chunk &ch, const std
                     const size_t eo = v.size();
                     v.resize(eo + 16, 0);
                     put(v, eo, t->eff_val[e]);
-                    put(v, eo + 8, row_of(t->eff_idx[e]));
+                    put(v, eo + 8, d_of(t->eff_idx[e]));
+                    put(v, eo + 12, u_of(t->eff_idx[e]));
                 }
             }
-            put(v, o + 24, x0);
-            put(v, o + 28, x1);
-            put(v, o + 32, row_of(B.slot(t->reac, 0, r)));
-            put(v, o + 36, row_of(B.slot(t->reac, 1, r)));
-            put(v, o + 40, row_of(B.slot(t->prod, 0, r)));
-            put(v, o + 44, row_of(B.slot(t->prod, 1, r)));
+            put(v, o + 48, x0);
+            put(v, o + 52, x1);
+            put(v, o + 56, u_of(B.slot(t->reac, 2, r)));
+            put(v, o + 60, u_of(B.slot(t->prod, 2, r)));
             if (B.kind(r) == 2) {
                 const int i2 = r - B.Ne - B.N3;
                 const double q[8] = {crf::kLog2e * t->lnA0[i2], crf::kLog2e * t->beta0[i2], -crf::kLog2e * t->Ea0_R[i2],
@@ -213,30 +223,36 @@ std::vector<unsigned char> chunk_block(const Mech &B, const Chunk &ch, const std
         put(v, 32 * (size_t)w + 12, (unsigned)troe0);
         for (int c = 0; c < 4; ++c) put(v, 32 * (size_t)w + 16 + 2 * (size_t)c, cnt[c]);
     }
-    // incidence entries per warp: slot-major, u32 = byte offset of the q row | sign << 31; |nu| = 2 -> two entries
-    (void)Rc;
+    // incidence lists per warp, slot-major: plus list then minus list of each owned species, u32 = byte offset of the q
+    // row (|nu| = 2 -> two entries), each list padded to even length with the zero row (row Rc)
     for (int w = 0; w < W; ++w) {
         align16();
         const size_t tab = v.size();
-        v.resize(tab + 4 * ((size_t)maxown + 4), 0);  // end[maxown], start, pad
+        v.resize(tab + 8 * (size_t)maxown + 16, 0);  // {endP, endM}[maxown], start, pad
         put(v, 32 * (size_t)w + 8, (unsigned)tab);
-        put(v, tab + 4 * (size_t)maxown, (unsigned)v.size());
+        put(v, tab + 8 * (size_t)maxown, (unsigned)v.size());
         for (int sl = 0; sl < maxown; ++sl) {
             const int k = own[(size_t)w * maxown + sl];
-            v.resize((v.size() + 7) & ~size_t(7), 0);  // a list starts 8-byte aligned (entries are read two at a time)
-            if (k >= 0)
-                for (int r : ch.rx) {
-                    const int nu = B.nu(r, k);
-                    for (int c = 0; c < std::abs(nu); ++c) {
-                        const size_t eo = v.size();
-                        v.resize(eo + 4, 0);
-                        put(v, eo, (unsigned)qrow[r] * rowb | (nu < 0 ? 0x80000000u : 0u));
+            for (int sign = +1; sign >= -1; sign -= 2) {
+                int cnt = 0;
+                if (k >= 0)
+                    for (int r : ch.rx) {
+                        const int nu = B.nu(r, k);
+                        for (int c = 0; c < std::abs(nu) && nu * sign > 0; ++c, ++cnt) {
+                            const size_t eo = v.size();
+                            v.resize(eo + 4, 0);
+                            put(v, eo, (unsigned)qrow[r] * rowb);
+                        }
                     }
+                if (cnt & 1) {
+                    const size_t eo = v.size();
+                    v.resize(eo + 4, 0);
+                    put(v, eo, (unsigned)Rc * rowb);
                 }
-            put(v, tab + 4 * (size_t)sl, (unsigned)v.size());
+                put(v, tab + 8 * (size_t)sl + (sign > 0 ? 0 : 4), (unsigned)v.size());
+            }
         }
     }
-    v.resize(v.size() + 16, 0);  // (the entry loop may read one 8-byte pair past the last list)
     align16();
     return v;
 }
@@ -274,27 +290,40 @@ RatesGroupPlanOffsets build_rates_group_plan(const crf_tables *t, const crf_plan
     const int own_n = (Ns + W - 1) / W, maxown = own_n <= 4 ? 4 : (own_n <= 8 ? 8 : 16);
     const std::vector<int> own = deal_species(B, W, maxown);
 
-    // Chunks: as few as the q buffer allows ((Rc + 1) rows of 256 PPL bytes next to the state and two stage buffers)
-    const size_t fixed = state(PPL) + 256;  // + mbarriers, chunk descriptors
+    // U in tensor memory (rates_group.cu): 2 PPL columns per species (+ the dummy species), a power of two >= 32 per
+    // block, and the 16/W blocks an SM holds must fit the 512 columns together
+    int tm_cols = 32;
+    while (tm_cols < 2 * PPL * (Ns + 1)) tm_cols *= 2;
+    const bool tm_fits = tm_cols <= 512 && (16 / W) * tm_cols <= 512;
+    if (opt.rates_tmem == 2 && !tm_fits) return o;
+    const bool tm = opt.rates_tmem == 1 ? false : tm_fits;
+    if (!tm) tm_cols = 0;
+
+    // Chunks: as few as the q buffer allows (Rc + 1 rows of 256 PPL bytes next to the state and two stage buffers; with
+    // U in tensor memory the prologue also passes the u rows through the q buffer: W + Ns + 1 rows)
+    const size_t fixed = (tm ? state(PPL) / 2 : state(PPL)) + 1536;  // + mbarriers, chunk descriptors
     std::vector<Chunk> chunks;
     std::vector<std::vector<unsigned char>> blocks;
     size_t stage_bytes = 0;
-    int Rc = 0;
+    int Rc = 0, q_rows = 0;
     const int first = opt.rates_Rc > 0 ? std::max(1, (Nr + opt.rates_Rc - 1) / opt.rates_Rc) : 1;
     for (int n_chunks = first;; ++n_chunks) {
         if (n_chunks > 64 || n_chunks > Nr) return o;  // does not fit at all
         chunks = make_chunks(B, n_chunks, W);
         Rc = 0;
         for (const Chunk &c : chunks) Rc = std::max(Rc, (int)c.rx.size());
+        q_rows = std::max(Rc + 1, tm ? W + Ns + 1 : W);
         blocks.clear();
         stage_bytes = 0;
         for (const Chunk &c : chunks) {
-            blocks.push_back(chunk_block(B, c, own, PPL, W, maxown, Rc));
+            blocks.push_back(chunk_block(B, c, own, PPL, W, maxown, Rc, tm));
             stage_bytes = std::max(stage_bytes, blocks.back().size());
         }
         stage_bytes = std::max(stage_bytes, (size_t)128 * Ns);  // the buffers also carry the NASA sets (prologue, epilogue)
-        if (fixed + (size_t)(Rc + 1) * 256 * PPL + 2 * stage_bytes <= budget(W)) break;
+        if (fixed + (size_t)q_rows * 256 * PPL + 2 * stage_bytes <= budget(W)) break;
     }
+    o.q_rows = q_rows, o.tm_cols = tm_cols;
+    o.log2_c0 = std::log2(t->p_ref / CRF_R_GAS);
     o.W = W, o.PPL = PPL, o.maxown = maxown, o.Rc = Rc;
     o.n_chunks = (int)chunks.size(), o.stage_bytes = (int)stage_bytes;
 

@@ -158,7 +158,6 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, const crf_plan_o
     const int Ns = B.Ns, Nr = B.Nr;
     const int want = opt.rates_kernel;
     if (Nr == 0 || Ns > 256 || want == CRF_RATES_STAGED || want == CRF_RATES_GENERIC || want == CRF_RATES_GROUP) return o;
-    if (want == CRF_RATES_AUTO && Ns > 12) return o;  // the warp-group kernel (rates_group.cu)
     for (int r = B.Ne; r < Nr; ++r)
         if (B.generic(r)) return o;  // a third body next to three explicit reactants: staged kernel
     if (!product_form_in_range(B)) return o;
@@ -179,46 +178,7 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, const crf_plan_o
         }
         if (stage_bytes <= 24 * 1024) o.W = 1, o.PPL = 4, o.maxown = 4, o.Rc = 0;
     }
-    if (want == CRF_RATES_THREAD && o.W == 0) return o;  // unsupported request
-    if (o.W == 0) {
-    // warps per point group W and points per lane PPL: 16 warps per SM, so a block may use 1/(16/W) of the
-    // SM's shared memory; the (C, d) state of its 32 PPL points should leave room for the q buffer and the
-    // two chunk blocks.  crf_plan_options.rates_W / rates_PPL / rates_Rc override.
-    auto budget = [](int W) { return (size_t)233472 / (16 / W) - 1024; };
-    auto state = [&](int PPL) { return (size_t)(Ns + 1) * 512 * PPL; };
-    // Measured (rates, ms): C5 W/PPL 16/2 11.0, 8/1 13.8, 16/1 14.4; C4 8/2 9.0, 16/2 10.9, 8/1 13.0, 4/2 21.0;
-    // C3 4/2 2.6, 8/2 3.0, 4/1 4.2; C2 4/2 3.4, 4/1 5.5 -> two points per lane whenever the state fits, and the
-    // fewest warps whose share of the SM's shared memory holds the state with room for the q buffer.
-    auto pick_w = [&](int ppl) {
-        for (int w = 4; w <= 16; w *= 2)
-            if (state(ppl) <= budget(w) * 6 / 10 && (Ns + w - 1) / w <= 16) return w;
-        return 0;
-    };
-    int PPL = opt.rates_PPL ? opt.rates_PPL : (pick_w(2) ? 2 : 1);
-    if (PPL != 1 && PPL != 2) PPL = 1;
-    int W = opt.rates_W;
-    if (W != 4 && W != 8 && W != 16) W = pick_w(PPL) ? pick_w(PPL) : 16;
-    if ((Ns + W - 1) / W > 16 || state(PPL) + 2 * W * 256 * PPL > budget(W)) return o;
-
-    const int own = (Ns + W - 1) / W, maxown = own <= 4 ? 4 : (own <= 8 ? 8 : 16);
-    const int step = 2 * W;
-    int Rc = opt.rates_Rc;
-    for (int cand = Rc > 0 ? (Rc + step - 1) / step * step : std::min(256, (Nr + step - 1) / step * step);
-         cand >= step; cand -= step) {
-        chunks = make_chunks(B, cand);
-        blocks.clear();
-        stage_bytes = 0;
-        for (const Chunk &ch : chunks) {
-            blocks.push_back(chunk_block(B, ch, PPL, W, maxown));
-            stage_bytes = std::max(stage_bytes, (blocks.back().size() + 15) & ~size_t(15));
-        }
-        stage_bytes = std::max(stage_bytes, (size_t)128 * Ns);  // the buffers also carry the NASA sets (prologue, epilogue)
-        Rc = cand;
-        if (state(PPL) + (size_t)cand * 256 * PPL + 2 * stage_bytes <= budget(W)) break;
-        if (cand == step) return o;  // does not fit at all
-    }
-    o.W = W, o.PPL = PPL, o.maxown = maxown, o.Rc = Rc;
-    }
+    if (o.W == 0) return o;  // (larger mechanisms: rates_group.cu)
     if (chunks.size() > 64) return RatesSmemPlanOffsets();  // the kernel keeps at most 64 chunk descriptors
     o.n_chunks = (int)chunks.size(), o.stage_bytes = (int)stage_bytes;
 

@@ -2,24 +2,29 @@
 // mechanism admits its plan (plan_rates_group.cu); rates_staged.cu (log-space K_c) and rates.cu are the fall-backs.
 //
 // Shape.  W warps share a group of 32 PPL grid points (lane = point, PPL points per lane), so every mechanism
-// coefficient is a warp-uniform shared-memory load.  The kernel is bound by two resources at once, the FP64 pipe and
-// the shared-memory pipe (128 bytes per cycle per SM), so both the FP64 instructions and the shared-memory bytes per
-// reaction are kept as low as the method allows:
+// coefficient is a warp-uniform shared-memory load.  ncu (profiles/r02_rates_c5.md) shows the kernel bound by two
+// resources at once, the issue port (FP64 instructions hold it for two cycles) and the shared-memory pipe (one
+// 128-byte wavefront per cycle per SM), so the FP64 instructions and the shared-memory bytes per reaction are both kept
+// as low as the method allows, and part of the state lives in TENSOR MEMORY, which has its own read path:
 //
 //   activity form   per point and species the block keeps d_k = (p_ref/RT) exp(-g_k/RT) and u_k = C_k / d_k.
 //                   With K_c = prod_products d / prod_reactants d, k_r = k_f / K_c and
 //                   C_k = u_k d_k the rate of progress of step 8 becomes
 //                       q = k_f prod_reactants d_a (prod_reactants u_a - prod_products u_b) [M]
-//                   one exponential (k_f) per reaction, no division, and the product side needs u only: 96 bytes of
-//                   state per reaction and two points instead of 128.  crf_mech_create admits this form only if every
-//                   factor stays a normal double for 250 K <= T <= 5000 K (plan_rates_group.cu).
-//   pair layout     the PPL = 2 points of a lane are adjacent in every row (state rows U_k, D_k, q rows): one 128-bit
-//                   access serves both.
+//                   one exponential (k_f) per reaction, no division, and the product side needs u only.
+//                   crf_mech_create admits this form only if every factor stays a normal double for
+//                   250 K <= T <= 5000 K (plan_rates_group.cu).
+//   U in TMEM       (TM = true, Ns <= 127 at two points per lane) the u rows, four of the six state rows a reaction
+//                   reads, live in tensor memory: lane = grid point pair, 2 PPL columns per species, read with
+//                   tcgen05.ld.32x32b (a warp reads the lanes of its own quadrant, so the prologue replicates U into the
+//                   quadrants of all warps); only the d rows, the q buffer and the chunk tables use shared memory.
+//   pair layout     the PPL = 2 points of a lane are adjacent in every row: one 128-bit access serves both.
 //   reaction stage  the reactions are cut into a few chunks; a chunk's reactions are dealt to the warps balanced by
 //                   cost (a falloff reaction costs six elementary ones), q_r -> q buffer.
-//   species stage   every species is owned by one warp (balanced by incidence count); the owner sums nu_kr q_r over the
-//                   chunk's incidence list of the species (4-byte entries: q row | sign) into register accumulators
-//                   that live for the whole kernel: omega never touches shared memory.
+//   species stage   every species is owned by one warp (balanced by incidence count); the owner sums q_r over the
+//                   chunk's plus list and minus list of the species (4-byte entries = q row offsets, read two at a time,
+//                   lists padded to even length with the zero row) into register accumulators that live for the whole
+//                   kernel: omega never touches shared memory.
 //   staging         a chunk's tables (records, Troe sets, third-body lists, incidence lists) are one contiguous block,
 //                   copied global -> shared by ONE bulk copy (cp.async.bulk, completion on an mbarrier) issued by one
 //                   thread while the previous chunk is evaluated.
@@ -153,43 +158,141 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
         : "memory");
 }
 
+// ---- tensor memory as per-lane storage: lane = this thread's lane of the warp's quadrant, 32-bit columns ---------------
+// A row of PPL doubles is 2 PPL columns.  Loads are asynchronous: the registers are valid after tm_wait, which takes
+// them as operands so that no use can be scheduled before it.
+template <int PPL>
+struct TmRow {
+    unsigned r[2 * PPL];
+};
+template <int PPL>
+__device__ __forceinline__ void tm_ld(unsigned taddr, TmRow<PPL> &t)
+{
+    if (PPL == 2)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(t.r[0]), "=r"(t.r[1]), "=r"(t.r[2 * PPL - 2]), "=r"(t.r[2 * PPL - 1])
+                     : "r"(taddr));
+    else
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(t.r[0]), "=r"(t.r[1]) : "r"(taddr));
+}
+template <int PPL>
+__device__ __forceinline__ void tm_st(unsigned taddr, const double (&v)[PPL])
+{
+    if (PPL == 2)
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(__double2loint(v[0])),
+                     "r"(__double2hiint(v[0])), "r"(__double2loint(v[PPL - 1])), "r"(__double2hiint(v[PPL - 1]))
+                     : "memory");
+    else
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(__double2loint(v[0])),
+                     "r"(__double2hiint(v[0]))
+                     : "memory");
+}
+template <int PPL>
+__device__ __forceinline__ void tm_wait1(TmRow<PPL> &a)
+{
+    if (PPL == 2)
+        asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(a.r[0]), "+r"(a.r[1]), "+r"(a.r[2 * PPL - 2]), "+r"(a.r[2 * PPL - 1]));
+    else
+        asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(a.r[0]), "+r"(a.r[1]));
+}
+template <int PPL>
+__device__ __forceinline__ void tm_get(const TmRow<PPL> &t, double (&v)[PPL])
+{
+#pragma unroll
+    for (int u = 0; u < PPL; ++u) v[u] = __hiloint2double((int)t.r[2 * u + 1], (int)t.r[2 * u]);
+}
+
+// the u row of one species: from tensor memory (h = column) or from shared memory (h = byte offset in the state)
+template <bool TM, int PPL>
+struct URow {
+    TmRow<PPL> t;
+    double v[PPL];
+    __device__ __forceinline__ void load(const char *sl, unsigned tmq, unsigned h)
+    {
+        if (TM)
+            tm_ld<PPL>(tmq + h, t);
+        else
+            ld_row<PPL>(sl + h, v);
+    }
+    __device__ __forceinline__ void get(double (&o)[PPL])
+    {
+        if (TM) {
+            tm_get<PPL>(t, o);
+        } else {
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) o[u] = v[u];
+        }
+    }
+};
+// one wait for up to six rows in flight (a wait covers every earlier load of the thread; the operands order the uses)
+template <bool TM, int PPL>
+__device__ __forceinline__ void u_wait(URow<TM, PPL> &a, URow<TM, PPL> &b, URow<TM, PPL> &c, URow<TM, PPL> &d)
+{
+    if (!TM) return;
+    if (PPL == 2)
+        asm volatile("tcgen05.wait::ld.sync.aligned;"
+                     : "+r"(a.t.r[0]), "+r"(a.t.r[1]), "+r"(a.t.r[2 * PPL - 2]), "+r"(a.t.r[2 * PPL - 1]), "+r"(b.t.r[0]),
+                       "+r"(b.t.r[1]), "+r"(b.t.r[2 * PPL - 2]), "+r"(b.t.r[2 * PPL - 1]), "+r"(c.t.r[0]), "+r"(c.t.r[1]),
+                       "+r"(c.t.r[2 * PPL - 2]), "+r"(c.t.r[2 * PPL - 1]), "+r"(d.t.r[0]), "+r"(d.t.r[1]),
+                       "+r"(d.t.r[2 * PPL - 2]), "+r"(d.t.r[2 * PPL - 1]));
+    else
+        asm volatile("tcgen05.wait::ld.sync.aligned;"
+                     : "+r"(a.t.r[0]), "+r"(a.t.r[1]), "+r"(b.t.r[0]), "+r"(b.t.r[1]), "+r"(c.t.r[0]), "+r"(c.t.r[1]),
+                       "+r"(d.t.r[0]), "+r"(d.t.r[1]));
+}
+
 template <int PPL>
 struct Ctx {
     double T[PPL], L[PPL], rT[PPL];  // T, ln T, 1/T
     double Csum[PPL];                // p/(R T)
 };
 
-// q of one reaction at the PPL points of this lane.  rec: the 48-byte record; tr: its Troe set (kind 2); blk: the chunk
-// block (third-body lists); sl: the state at this lane (row offsets come from the record; D_k is RB bytes behind U_k).
-template <int KIND, bool GENERIC, int PPL>
-__device__ __forceinline__ void reaction_q(const char *blk, const char *rec, const char *tr, const char *sl,
+// q of one reaction at the PPL points of this lane.  rec: the 64-byte record; tr: its Troe set (kind 2); blk: the chunk
+// block (third-body lists); sl: the shared-memory state at this lane (d rows; the u rows too unless TM); tmq: the
+// tensor-memory address of this warp's quadrant.
+template <int KIND, bool GENERIC, int PPL, bool TM>
+__device__ __forceinline__ void reaction_q(const char *blk, const char *rec, const char *tr, const char *sl, unsigned tmq,
                                            const Ctx<PPL> &c, double (&q)[PPL])
 {
-    constexpr int RB = 256 * PPL;
     const double2 A = lds2(rec);        // log2e lnA, log2e beta
-    const double2 Ex = lds2(rec + 16);  // -log2e Ea/R, (x0, x1)
-    const uint4 S = ldsu4(rec + 32);    // a0, a1, b0, b1
-    const unsigned x0 = (unsigned)__double2loint(Ex.y), x1 = (unsigned)__double2hiint(Ex.y);
-    double ua0[PPL], ua1[PPL], da0[PPL], da1[PPL], ub0[PPL], ub1[PPL];
-    ld_row<PPL>(sl + S.x, ua0), ld_row<PPL>(sl + S.x + RB, da0);
-    ld_row<PPL>(sl + S.y, ua1), ld_row<PPL>(sl + S.y + RB, da1);
-    ld_row<PPL>(sl + S.z, ub0), ld_row<PPL>(sl + S.w, ub1);
+    const double2 Ex = lds2(rec + 16);  // -log2e Ea/R, (b0u, b1u)
+    const uint4 S = ldsu4(rec + 32);    // a0d, a1d, a0u, a1u
+    const unsigned b0u = (unsigned)__double2loint(Ex.y), b1u = (unsigned)__double2hiint(Ex.y);
+    URow<TM, PPL> Ua0, Ua1, Ub0, Ub1;
+    Ua0.load(sl, tmq, S.z), Ua1.load(sl, tmq, S.w), Ub0.load(sl, tmq, b0u), Ub1.load(sl, tmq, b1u);
+    double da0[PPL], da1[PPL];
+    ld_row<PPL>(sl + S.x, da0), ld_row<PPL>(sl + S.y, da1);
+    uint4 X = make_uint4(0, 0, 0, 0);  // x0, x1, x0u, x1u
+    if (KIND != 0 || GENERIC) X = ldsu4(rec + 48);
+    u_wait<TM, PPL>(Ua0, Ua1, Ub0, Ub1);
+    double ua0[PPL], ua1[PPL], ub0[PPL], ub1[PPL];
+    Ua0.get(ua0), Ua1.get(ua1), Ub0.get(ub0), Ub1.get(ub1);
     double M[PPL];
     if (KIND != 0) {
 #pragma unroll
         for (int u = 0; u < PPL; ++u) M[u] = c.Csum[u];
-        const char *e = blk + x0, *e1 = e + 16 * x1;
+        const char *e = blk + X.x, *e1 = e + 16 * X.y;
         for (; e < e1; e += 16) {
-            const uint4 en = ldsu4(e);
+            const uint4 en = ldsu4(e);  // f64 efficiency - 1, u32 d row, u32 u handle
             const double coef = __hiloint2double((int)en.y, (int)en.x);
+            URow<TM, PPL> Uk;
+            Uk.load(sl, tmq, en.w);
             double uu[PPL], dd[PPL];
-            ld_row<PPL>(sl + en.z, uu), ld_row<PPL>(sl + en.z + RB, dd);
+            ld_row<PPL>(sl + en.z, dd);
+            if (TM) tm_wait1<PPL>(Uk.t);
+            Uk.get(uu);
 #pragma unroll
             for (int u = 0; u < PPL; ++u) M[u] = fma(coef, uu[u] * dd[u], M[u]);  // C_k = u_k d_k
         }
     }
     double ua2[PPL], da2[PPL], ub2[PPL];
-    if (GENERIC) ld_row<PPL>(sl + x0, ua2), ld_row<PPL>(sl + x0 + RB, da2), ld_row<PPL>(sl + x1, ub2);
+    if (GENERIC) {
+        URow<TM, PPL> Ua2, Ub2;
+        Ua2.load(sl, tmq, X.z), Ub2.load(sl, tmq, X.w);
+        ld_row<PPL>(sl + X.x, da2);
+        if (TM) tm_wait1<PPL>(Ua2.t), tm_wait1<PPL>(Ub2.t);
+        Ua2.get(ua2), Ub2.get(ub2);
+    }
 #pragma unroll
     for (int u = 0; u < PPL; ++u) {
         const double yinf = fma(A.y, c.L[u], fma(Ex.x, c.rT[u], A.x));  // log2 k_f (high-pressure limit)
@@ -224,33 +327,58 @@ __device__ __forceinline__ void reaction_q(const char *blk, const char *rec, con
     }
 }
 
-template <int KIND, bool GENERIC, int PPL>
+template <int KIND, bool GENERIC, int PPL, bool TM>
 __device__ __forceinline__ void reaction_loop(const char *blk, const char *&rec, const char *&tr, char *&qp, int count,
-                                              const char *sl, const Ctx<PPL> &c)
+                                              const char *sl, unsigned tmq, const Ctx<PPL> &c)
 {
     constexpr int RB = 256 * PPL;
 #pragma unroll 1
     for (int i = 0; i < count; ++i) {
         double q[PPL];
-        reaction_q<KIND, GENERIC, PPL>(blk, rec, tr, sl, c, q);
+        reaction_q<KIND, GENERIC, PPL, TM>(blk, rec, tr, sl, tmq, c, q);
         st_row<PPL>(qp, q);
-        rec += 48, qp += RB;
+        rec += 64, qp += RB;
         if (KIND == 2) tr += 64;
     }
 }
 
-// one incidence entry: om += (+-1) q[row]
-template <int PPL>
-__device__ __forceinline__ void gather(unsigned en, const char *sQl, double (&om)[PPL])
+// om (+/-)= q[row a] + q[row b]
+template <int PPL, bool PLUS>
+__device__ __forceinline__ void gather2(uint2 en, const char *sQl, double (&om)[PPL])
 {
-    double q[PPL];
-    ld_row<PPL>(sQl + (en & 0x7fffffffu), q);
-    const double nu = __hiloint2double((int)((en & 0x80000000u) | 0x3ff00000u), 0);
+    double qa[PPL], qb[PPL];
+    ld_row<PPL>(sQl + en.x, qa), ld_row<PPL>(sQl + en.y, qb);
 #pragma unroll
-    for (int u = 0; u < PPL; ++u) om[u] = fma(nu, q[u], om[u]);
+    for (int u = 0; u < PPL; ++u) om[u] = PLUS ? (om[u] + qa[u]) + qb[u] : (om[u] - qa[u]) - qb[u];
+}
+// one list [e, end): 8-byte aligned, even length
+template <int PPL, bool PLUS>
+__device__ __forceinline__ void gather_list(const char *blk, unsigned &e, unsigned end, const char *sQl, double (&om)[PPL])
+{
+#pragma unroll 1
+    for (; e < end; e += 8) gather2<PPL, PLUS>(ldsu2(blk + e), sQl, om);
 }
 
-template <int W, int PPL, int MAXOWN>
+// g/(RT) set (log2 e folded in) or h/(RT) set of one species at one point: 7 (6) Horner coefficients of the range T is in,
+// read with a per-lane address (the two ranges are 64 bytes apart: lanes in different ranges hit different banks)
+template <bool GIBBS>
+__device__ __forceinline__ double nasa_eval(const double2 *set, double Tu, double rTu, double omL, double Tmid)
+{
+    const double2 *g = set + (Tu <= Tmid ? 0 : 4);
+    const double2 c01 = g[0], c23 = g[1], c45 = g[2];
+    double v = fma(Tu, c45.x, c23.y);
+    v = fma(Tu, v, c23.x);
+    v = fma(Tu, v, c01.y);
+    if (GIBBS) {
+        v = fma(Tu, v, g[3].x);
+        v = fma(c45.y, rTu, v);
+        return fma(c01.x, omL, v);  // c0 (1 - ln T)
+    }
+    v = fma(Tu, v, c01.x);
+    return fma(c45.y, rTu, v);
+}
+
+template <int W, int PPL, int MAXOWN, bool TM>
 __global__ void __launch_bounds__(32 * W, 16 / W)
     rates_group_kernel(DevTables m, const double *__restrict__ T, const double *__restrict__ p,
                        const double *__restrict__ Y, int64_t n, double *__restrict__ omega, double *__restrict__ qdot)
@@ -258,13 +386,15 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     extern __shared__ double2 sm2[];
     __shared__ uint64_t mbar[2];
     __shared__ int4 sChunk[64];
+    __shared__ unsigned sTmBase;
     const RatesGroupPlan &rg = m.rg;
     constexpr int RB = 256 * PPL, LB = 8 * PPL;
     const int Ns = m.Ns;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    char *sS = reinterpret_cast<char *>(sm2);                 // [Ns + 1][2][RB] (U_k, D_k); row Ns = (1, 1)
-    char *sQ = sS + (size_t)(Ns + 1) * 2 * RB;                // [max(Rc, W)][RB] q_r; also the reduction scratch
-    char *sStage = sQ + (size_t)max(rg.Rc, W) * RB;           // [2][stage_bytes]
+    // state rows: TM: [Ns + 1] d rows; otherwise [Ns + 1] d rows then [Ns + 1] u rows; row Ns = 1 (the dummy species)
+    char *sS = reinterpret_cast<char *>(sm2);
+    char *sQ = sS + (size_t)(Ns + 1) * (TM ? 1 : 2) * RB;  // [q_rows][RB] q_r (row Rc = 0); prologue scratch
+    char *sStage = sQ + (size_t)rg.q_rows * RB;            // [2][stage_bytes]
     char *sl = sS + lane * LB;
     char *sQl = sQ + lane * LB;
     const int sb = rg.stage_bytes, nch = rg.n_chunks;
@@ -274,13 +404,22 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         mbar_init(&mbar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (TM && warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sTmBase)),
+                     "r"((unsigned)rg.tm_cols)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
     for (int ci = threadIdx.x; ci < nch && ci < 64; ci += 32 * W) sChunk[ci] = __ldg(rg.chunk + ci);
+    if (TM) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (TM) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     if (threadIdx.x == 0) {
         // chunk 0 -> buffer 0; buffer 1 is free until chunk 1 is prefetched: it carries the g/(RT) sets for the prologue
         bulk_load(sStage, rg.stage + sChunk[0].x, (unsigned)sChunk[0].y, &mbar[0]);
         bulk_load(sStage + sb, rg.gco, 128u * Ns, &mbar[1]);
     }
+    const unsigned tmq = TM ? sTmBase + (((unsigned)(warp & 3) * 32u) << 16) : 0u;
 
     const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * PPL;
     const bool vec = (n & 1) == 0;
@@ -295,12 +434,13 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         const int k = warp + W * s;
         if (k < Ns) load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, z[s]);
     }
-    double lc02[PPL];
+    double lc02[PPL], omL[PPL];
 #pragma unroll
     for (int u = 0; u < PPL; ++u) {
         c.L[u] = log(c.T[u]);
         c.rT[u] = 1.0 / c.T[u];
-        lc02[u] = crf::kLog2e * (log(m.p_ref / CRF_R_GAS) - c.L[u]);  // log2(p_ref/(R T))
+        lc02[u] = fma(-crf::kLog2e, c.L[u], rg.log2_c0);  // log2(p_ref/(R T))
+        omL[u] = 1.0 - c.L[u];
         c.Csum[u] = pi[u] * c.rT[u] * (1.0 / CRF_R_GAS);
     }
     mbar_wait(&mbar[1], 0);
@@ -320,7 +460,8 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
             }
         }
     }
-    double *sred = reinterpret_cast<double *>(sQ);  // [W][PPL][32], valid outside the chunk loop
+    double *sred = reinterpret_cast<double *>(sQ);  // rows [0, W): [W][PPL][32] reduction scratch, outside the chunk loop
+    char *sUtmp = sQ + (size_t)W * RB;               // TM: rows [W, W + Ns + 1): the u rows on their way to tensor memory
 #pragma unroll
     for (int u = 0; u < PPL; ++u) sred[(warp * PPL + u) * 32 + lane] = invW[u];
     __syncthreads();
@@ -333,44 +474,49 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         rho[u] = pi[u] / (CRF_R_GAS * c.T[u] * s);
     }
     // ---- a2: d_k = 2^(log2(p_ref/RT) - log2e g_k/RT), u_k = rho Z_k / d_k
+    char *uDst = (TM ? sUtmp : sS + (size_t)(Ns + 1) * RB) + lane * LB;
 #pragma unroll
     for (int s = 0; s < MAXOWN; ++s) {
         const int k = warp + W * s;
         if (k >= Ns) continue;
         const double2 *g = sG + 8 * k;
-        const double2 l01 = g[0], l23 = g[1], l45 = g[2], l6t = g[3];
-        const double2 h01 = g[4], h23 = g[5], h45 = g[6], h6w = g[7];
+        const double Tmid = g[3].y;
         double uu[PPL], dd[PPL];
 #pragma unroll
         for (int u = 0; u < PPL; ++u) {
-            const double Tu = c.T[u], oml = 1.0 - c.L[u];
-            double lo = fma(Tu, l45.x, l23.y);
-            lo = fma(Tu, lo, l23.x);
-            lo = fma(Tu, lo, l01.y);
-            lo = fma(Tu, lo, l6t.x);
-            lo = fma(l45.y, c.rT[u], lo);
-            lo = fma(l01.x, oml, lo);
-            double hi = fma(Tu, h45.x, h23.y);
-            hi = fma(Tu, hi, h23.x);
-            hi = fma(Tu, hi, h01.y);
-            hi = fma(Tu, hi, h6w.x);
-            hi = fma(h45.y, c.rT[u], hi);
-            hi = fma(h01.x, oml, hi);
-            const double g2 = Tu <= l6t.y ? lo : hi;
+            const double g2 = nasa_eval<true>(g, c.T[u], c.rT[u], omL[u], Tmid);
             dd[u] = exp2r(lc02[u] - g2);
             uu[u] = (rho[u] * z[s][u]) * rcp_fast(dd[u]);
         }
-        st_row<PPL>(sl + (size_t)k * 2 * RB, uu);
-        st_row<PPL>(sl + (size_t)k * 2 * RB + RB, dd);
+        st_row<PPL>(uDst + (size_t)k * RB, uu);
+        st_row<PPL>(sl + (size_t)k * RB, dd);
     }
     if (warp == 0) {
         double one[PPL];
 #pragma unroll
         for (int u = 0; u < PPL; ++u) one[u] = 1.0;
-        st_row<PPL>(sl + (size_t)Ns * 2 * RB, one);
-        st_row<PPL>(sl + (size_t)Ns * 2 * RB + RB, one);
+        st_row<PPL>(uDst + (size_t)Ns * RB, one);
+        st_row<PPL>(sl + (size_t)Ns * RB, one);
     }
     __syncthreads();  // the state is complete; everyone is done with the g sets and the reduction scratch
+    if (TM) {
+        // every quadrant gets the whole of U: the W/4 warps of a quadrant split the rows
+        for (int k = warp >> 2; k <= Ns; k += W / 4) {
+            double uu[PPL];
+            ld_row<PPL>(sUtmp + (size_t)k * RB + lane * LB, uu);
+            tm_st<PPL>(tmq + (unsigned)(2 * PPL * k), uu);
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    }
+    if (warp == W - 1) {  // the zero row the padded incidence lists point at
+        double zero[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) zero[u] = 0.0;
+        st_row<PPL>(sQl + (size_t)rg.Rc * RB, zero);
+    }
 
     double om[MAXOWN][PPL];
 #pragma unroll
@@ -393,30 +539,22 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
             const uint2 cn = ldsu2(blk + 32 * warp + 16);
             const char *rec = blk + hw.x, *tr = blk + hw.w;
             char *qp = sQl + hw.y;
-            reaction_loop<0, false, PPL>(blk, rec, tr, qp, (int)(cn.x & 0xffffu), sl, c);
-            if (cn.x >> 16) reaction_loop<0, true, PPL>(blk, rec, tr, qp, (int)(cn.x >> 16), sl, c);
-            if (cn.y & 0xffffu) reaction_loop<1, false, PPL>(blk, rec, tr, qp, (int)(cn.y & 0xffffu), sl, c);
-            if (cn.y >> 16) reaction_loop<2, false, PPL>(blk, rec, tr, qp, (int)(cn.y >> 16), sl, c);
+            reaction_loop<0, false, PPL, TM>(blk, rec, tr, qp, (int)(cn.x & 0xffffu), sl, tmq, c);
+            if (cn.x >> 16) reaction_loop<0, true, PPL, TM>(blk, rec, tr, qp, (int)(cn.x >> 16), sl, tmq, c);
+            if (cn.y & 0xffffu) reaction_loop<1, false, PPL, TM>(blk, rec, tr, qp, (int)(cn.y & 0xffffu), sl, tmq, c);
+            if (cn.y >> 16) reaction_loop<2, false, PPL, TM>(blk, rec, tr, qp, (int)(cn.y >> 16), sl, tmq, c);
             __syncthreads();
-            // ---- species stage: the warp's entries are contiguous (slot-major); slot s ends at end[s]
+            // ---- species stage: the warp's lists are contiguous: plus list of slot 0, minus list of slot 0, plus list of
+            // slot 1, ...; each 8-byte aligned and of even length; the table holds where each ends
             const char *tab = blk + hw.z;
-            unsigned e = *reinterpret_cast<const unsigned *>(tab + 4 * MAXOWN);
+            unsigned e = *reinterpret_cast<const unsigned *>(tab + 8 * MAXOWN);
 #pragma unroll
-            for (int s4 = 0; s4 < MAXOWN; s4 += 4) {
-                const uint4 ends = ldsu4(tab + 4 * s4);
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int s = s4 + j;
-                    const unsigned end = j == 0 ? ends.x : (j == 1 ? ends.y : (j == 2 ? ends.z : ends.w));
-#pragma unroll 1
-                    for (; e + 8 <= end; e += 8) {
-                        const uint2 en = ldsu2(blk + e);
-                        gather<PPL>(en.x, sQl, om[s]);
-                        gather<PPL>(en.y, sQl, om[s]);
-                    }
-                    if (e < end) gather<PPL>(*reinterpret_cast<const unsigned *>(blk + e), sQl, om[s]);
-                    e = (end + 7u) & ~7u;
-                }
+            for (int s2 = 0; s2 < MAXOWN; s2 += 2) {
+                const uint4 ends = ldsu4(tab + 8 * s2);  // endP[s2], endM[s2], endP[s2 + 1], endM[s2 + 1]
+                gather_list<PPL, true>(blk, e, ends.x, sQl, om[s2]);
+                gather_list<PPL, false>(blk, e, ends.y, sQl, om[s2]);
+                gather_list<PPL, true>(blk, e, ends.z, sQl, om[s2 + 1]);
+                gather_list<PPL, false>(blk, e, ends.w, sQl, om[s2 + 1]);
             }
         }
         __syncthreads();
@@ -433,23 +571,10 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         const int k = __ldg(rg.own + warp * MAXOWN + s);
         if (k >= 0) {
             const double2 *h = sH + 8 * k;
-            const double2 l01 = h[0], l23 = h[1], l45 = h[2], l6t = h[3];
-            const double2 h01 = h[4], h23 = h[5], h45 = h[6];
+            const double Tmid = h[3].y;
 #pragma unroll
-            for (int u = 0; u < PPL; ++u) {
-                const double Tu = c.T[u];
-                double lo = fma(Tu, l45.x, l23.y);
-                lo = fma(Tu, lo, l23.x);
-                lo = fma(Tu, lo, l01.y);
-                lo = fma(Tu, lo, l01.x);
-                lo = fma(l45.y, c.rT[u], lo);
-                double hi = fma(Tu, h45.x, h23.y);
-                hi = fma(Tu, hi, h23.x);
-                hi = fma(Tu, hi, h01.y);
-                hi = fma(Tu, hi, h01.x);
-                hi = fma(h45.y, c.rT[u], hi);
-                qd[u] = fma(-(Tu <= l6t.y ? lo : hi), om[s][u], qd[u]);
-            }
+            for (int u = 0; u < PPL; ++u)
+                qd[u] = fma(-nasa_eval<false>(h, c.T[u], c.rT[u], 0.0, Tmid), om[s][u], qd[u]);
             store_row<PPL>(omega + (int64_t)k * n, i0, n, vec, om[s]);
         }
     }
@@ -466,20 +591,23 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
             out[u] = s * (CRF_R_GAS * c.T[u]);
         }
         store_row<PPL>(qdot, i0, n, vec, out);
+        if (TM)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(sTmBase), "r"((unsigned)rg.tm_cols)
+                         : "memory");
     }
 }
 
-template <int W, int PPL, int MAXOWN>
+template <int W, int PPL, int MAXOWN, bool TM>
 cudaError_t launch_k(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
                      double *qdot, cudaStream_t st)
 {
     const size_t smem = rates_group_dynamic_smem(m);
-    cudaError_t e = cudaFuncSetAttribute(rates_group_kernel<W, PPL, MAXOWN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(rates_group_kernel<W, PPL, MAXOWN, TM>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int64_t per_block = 32 * PPL;
-    rates_group_kernel<W, PPL, MAXOWN><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, p, Y, n,
-                                                                                                         omega, qdot);
+    rates_group_kernel<W, PPL, MAXOWN, TM>
+        <<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, p, Y, n, omega, qdot);
     crf_count_launch();
     return cudaGetLastError();
 }
@@ -488,10 +616,13 @@ template <int W, int PPL>
 cudaError_t launch_wp(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
                       double *qdot, cudaStream_t st)
 {
-    switch (m.rg.maxown) {
-    case 4: return launch_k<W, PPL, 4>(m, T, p, Y, n, omega, qdot, st);
-    case 8: return launch_k<W, PPL, 8>(m, T, p, Y, n, omega, qdot, st);
-    case 16: return launch_k<W, PPL, 16>(m, T, p, Y, n, omega, qdot, st);
+    switch (m.rg.maxown * 2 + (m.rg.tm_cols > 0)) {
+    case 8: return launch_k<W, PPL, 4, false>(m, T, p, Y, n, omega, qdot, st);
+    case 9: return launch_k<W, PPL, 4, true>(m, T, p, Y, n, omega, qdot, st);
+    case 16: return launch_k<W, PPL, 8, false>(m, T, p, Y, n, omega, qdot, st);
+    case 17: return launch_k<W, PPL, 8, true>(m, T, p, Y, n, omega, qdot, st);
+    case 32: return launch_k<W, PPL, 16, false>(m, T, p, Y, n, omega, qdot, st);
+    case 33: return launch_k<W, PPL, 16, true>(m, T, p, Y, n, omega, qdot, st);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -502,7 +633,7 @@ size_t rates_group_dynamic_smem(const DevTables &m)
 {
     const RatesGroupPlan &rg = m.rg;
     const size_t rb = 256 * (size_t)rg.PPL;
-    return (size_t)(m.Ns + 1) * 2 * rb + (size_t)(rg.Rc > rg.W ? rg.Rc : rg.W) * rb + 2 * (size_t)rg.stage_bytes;
+    return (size_t)(m.Ns + 1) * (rg.tm_cols > 0 ? 1 : 2) * rb + (size_t)rg.q_rows * rb + 2 * (size_t)rg.stage_bytes;
 }
 
 cudaError_t launch_rates_group(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,

@@ -1,9 +1,7 @@
-// rates_smem.cu -- crf_production_rates, the kernel the library uses
-// whenever the mechanism admits its plan (plan_rates_smem.cu); rates_staged.cu / rates.cu are the fallbacks.
+// rates_smem.cu -- crf_production_rates for SMALL mechanisms: one thread per grid
+// point (plan_rates_smem.cu admits Ns <= 12 by default, up to 24 on request); larger mechanisms run rates_group.cu.
 //
-// Shape.  W warps share a group of 32 PPL grid points (lane = point, PPL points per lane), so every
-// mechanism coefficient is a warp-uniform shared-memory load.  Per point and species the block keeps
-// (C_k, d_k), d_k = (p_ref/RT) exp(-g_k/RT), in shared memory as [species][point] rows of double2.
+// Per point and species the thread keeps (C_k, d_k), d_k = (p_ref/RT) exp(-g_k/RT), as a column in shared memory.
 //
 //   k_f        = 2^(log2e lnA + log2e beta ln T - log2e Ea/(R T))                 one exponential per reaction
 //   1/K_c      = prod_reactants d / prod_products d                               (K_c = exp(-sum nu g/RT) (p_ref/RT)^dnu)
@@ -14,14 +12,8 @@
 // point.  crf_mech_create admits this form only if numerator, denominator and quotient stay inside the
 // double range for every T in [250, 5000] K (plan_rates_smem.cu), otherwise rates_staged.cu runs.
 //
-// Reactions are cut into chunks of one kind (elementary | third body | Troe falloff; two or three
-// species per side).  A chunk's tables (48-byte reaction records, per-species incidence lists, third-body
-// lists, Troe sets) are one contiguous block that the thread block copies global -> shared with cp.async
-// while it works on the previous chunk (double buffer), so the reaction loop never waits on L2.
-//   reaction stage: the warps split the reactions of the chunk, q_r -> sQ[r][point];
-//   species stage:  the warps split the SPECIES; each owned species sums nu_kr q_r over its incidence list
-//                   into register accumulators that live for the whole kernel (omega never touches
-//                   shared memory).
+// Reactions are cut into chunks of one kind (elementary | third body | Troe falloff; two or three species per side);
+// all chunk blocks (48-byte reaction records, third-body lists, Troe sets) are resident in shared memory.
 // Troe falloff is evaluated in base 2 (log2 F = log2 F_cent / (1 + f1^2)) with a branch-free logarithm.
 #include "crf_internal.h"
 #include "fastmath.cuh"
@@ -143,302 +135,6 @@ __device__ __forceinline__ void reaction_q(const char *blk, const char *rec, con
             q[u] = exp2c(yinf + l2F) * (Pred * rcp_fast(1.0 + Pred)) * net;
         }
     }
-}
-
-template <int W, int PPL, int KIND, bool GENERIC>
-__device__ __forceinline__ void reaction_stage(const char *blk, int count, int o_troe, const char *sL, char *sQl,
-                                               int warp, const Ctx<PPL> &c)
-{
-    constexpr int NRX = PPL == 1 ? 2 : 1;  // independent reactions per trip (ILP = NRX * PPL chains)
-    int rl = warp;
-    for (; rl + (NRX - 1) * W < count; rl += NRX * W) {
-        double q[NRX][PPL];
-#pragma unroll
-        for (int v = 0; v < NRX; ++v)
-            reaction_q<KIND, GENERIC, PPL>(blk, blk + 48 * (rl + v * W), blk + o_troe + 64 * (rl + v * W), sL, c, q[v]);
-#pragma unroll
-        for (int v = 0; v < NRX; ++v)
-#pragma unroll
-            for (int u = 0; u < PPL; ++u) *reinterpret_cast<double *>(sQl + (rl + v * W) * (256 * PPL) + 256 * u) = q[v][u];
-    }
-    if (NRX == 2 && rl < count) {
-        double q[PPL];
-        reaction_q<KIND, GENERIC, PPL>(blk, blk + 48 * rl, blk + o_troe + 64 * rl, sL, c, q);
-#pragma unroll
-        for (int u = 0; u < PPL; ++u) *reinterpret_cast<double *>(sQl + rl * (256 * PPL) + 256 * u) = q[u];
-    }
-}
-
-__device__ __forceinline__ void stage_async(char *dst, const unsigned char *src, int bytes, int tid, int nthreads)
-{
-    for (int o = tid * 16; o < bytes; o += nthreads * 16) {
-        const unsigned d = (unsigned)__cvta_generic_to_shared(dst + o);
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src + o) : "memory");
-    }
-    asm volatile("cp.async.commit_group;" ::: "memory");
-}
-__device__ __forceinline__ void stage_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
-// the PPL points of a lane are adjacent: i0, i0 + 1 (one 128-bit access per row when n is even)
-template <int PPL>
-__device__ __forceinline__ void load_row(const double *__restrict__ row, int64_t i0, int64_t n, bool vec, double (&v)[PPL])
-{
-    if (PPL == 2 && vec && i0 + 1 < n) {
-        const double2 t = *reinterpret_cast<const double2 *>(row + i0);
-        v[0] = t.x, v[PPL - 1] = t.y;
-    } else {
-#pragma unroll
-        for (int u = 0; u < PPL; ++u) v[u] = row[min(i0 + u, n - 1)];
-    }
-}
-template <int PPL>
-__device__ __forceinline__ void store_row(double *__restrict__ row, int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
-{
-    if (PPL == 2 && vec && i0 + 1 < n) {
-        *reinterpret_cast<double2 *>(row + i0) = make_double2(v[0], v[PPL - 1]);
-    } else {
-#pragma unroll
-        for (int u = 0; u < PPL; ++u)
-            if (i0 + u < n) row[i0 + u] = v[u];
-    }
-}
-
-template <int W, int PPL, int MAXOWN>
-__global__ void __launch_bounds__(32 * W, 16 / W)
-    rates_smem_kernel(DevTables m, const double *__restrict__ T, const double *__restrict__ p,
-                      const double *__restrict__ Y, int64_t n, double *__restrict__ omega, double *__restrict__ qdot)
-{
-    extern __shared__ double2 sm2[];
-    const RatesSmemPlan &rs = m.rs;
-    const int Ns = m.Ns;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    char *sCD = reinterpret_cast<char *>(sm2);                // [Ns + 1][PPL][32] (C_k, d_k); row Ns = (1, 1)
-    char *sQ = sCD + (size_t)(Ns + 1) * 512 * PPL;            // [Rc][PPL][32] q_r; also the reduction scratch
-    char *sStage = sQ + (size_t)rs.Rc * 256 * PPL;            // [2][stage_bytes]
-    char *sL = sCD + lane * 16;
-    char *sQl = sQ + lane * 8;
-    double *sred = reinterpret_cast<double *>(sQ);            // [W][PPL][32], valid outside the chunk loop
-
-    // chunk descriptors: read once, before the loop needs them (a global load at the top of every chunk would put
-    // an L2 round trip on every warp's critical path)
-    __shared__ int4 sChunk[64];
-    for (int ci = threadIdx.x; ci < rs.n_chunks && ci < 64; ci += 32 * W) sChunk[ci] = __ldg(rs.chunk + ci);
-    stage_async(sStage, rs.stage + __ldg(&rs.chunk[0].z), rs.stage_bytes, threadIdx.x, 32 * W);
-    // the second stage buffer is free until chunk 1 is prefetched: it carries the g/(RT) sets for the prologue
-    stage_async(sStage + rs.stage_bytes, reinterpret_cast<const unsigned char *>(rs.gco), 128 * Ns, threadIdx.x, 32 * W);
-
-    const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * PPL;
-    const bool vec = (n & 1) == 0;
-    Ctx<PPL> c;
-    double pi[PPL], lc02[PPL];
-    load_row<PPL>(T, i0, n, vec, c.T);
-    load_row<PPL>(p, i0, n, vec, pi);
-#pragma unroll
-    for (int u = 0; u < PPL; ++u) {
-        c.L[u] = log(c.T[u]);
-        c.rT[u] = 1.0 / c.T[u];
-        lc02[u] = crf::kLog2e * (log(m.p_ref / CRF_R_GAS) - c.L[u]);  // log2(p_ref/(R T))
-        c.Csum[u] = pi[u] * c.rT[u] * (1.0 / CRF_R_GAS);
-    }
-
-    stage_wait();
-    __syncthreads();
-    const double2 *sG = reinterpret_cast<const double2 *>(sStage + rs.stage_bytes);
-    // ---- a1, a2: Z_k = Y_k/W_k and d_k = 2^(log2(p_ref/RT) - log2e g_k/RT); warp w takes species w, w+W, ...
-    double invW[PPL];
-#pragma unroll
-    for (int u = 0; u < PPL; ++u) invW[u] = 0.0;
-    // (slots in groups of 4: the four Y row loads and the coefficient loads are in flight together)
-#pragma unroll
-    for (int s0 = 0; s0 < MAXOWN; s0 += 4) {
-        double y[4][PPL];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int k = warp + W * (s0 + j);
-            if (k < Ns) load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, y[j]);
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int k = warp + W * (s0 + j);
-            if (k >= Ns) continue;
-            const double2 *g = sG + 8 * k;
-            const double2 l01 = g[0], l23 = g[1], l45 = g[2], l6t = g[3];
-            const double2 h01 = g[4], h23 = g[5], h45 = g[6], h6w = g[7];
-#pragma unroll
-            for (int u = 0; u < PPL; ++u) {
-                const double Tu = c.T[u], oml = 1.0 - c.L[u];
-                double lo = fma(Tu, l45.x, l23.y);
-                lo = fma(Tu, lo, l23.x);
-                lo = fma(Tu, lo, l01.y);
-                lo = fma(Tu, lo, l6t.x);
-                lo = fma(l45.y, c.rT[u], lo);
-                lo = fma(l01.x, oml, lo);
-                double hi = fma(Tu, h45.x, h23.y);
-                hi = fma(Tu, hi, h23.x);
-                hi = fma(Tu, hi, h01.y);
-                hi = fma(Tu, hi, h6w.x);
-                hi = fma(h45.y, c.rT[u], hi);
-                hi = fma(h01.x, oml, hi);
-                const double g2 = Tu <= l6t.y ? lo : hi;
-                const double z = y[j][u] * h6w.y;
-                invW[u] += z;
-                *reinterpret_cast<double2 *>(sL + (size_t)k * 512 * PPL + 512 * u) = make_double2(z, exp2c(lc02[u] - g2));
-            }
-        }
-    }
-    if (warp == 0) {
-#pragma unroll
-        for (int u = 0; u < PPL; ++u)
-            *reinterpret_cast<double2 *>(sL + (size_t)Ns * 512 * PPL + 512 * u) = make_double2(1.0, 1.0);
-    }
-#pragma unroll
-    for (int u = 0; u < PPL; ++u) sred[(warp * PPL + u) * 32 + lane] = invW[u];
-    __syncthreads();
-    double rho[PPL];
-#pragma unroll
-    for (int u = 0; u < PPL; ++u) {
-        double s = 0.0;
-#pragma unroll
-        for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
-        rho[u] = pi[u] / (CRF_R_GAS * c.T[u] * s);
-    }
-    for (int k = warp; k < Ns; k += W) {
-#pragma unroll
-        for (int u = 0; u < PPL; ++u) *reinterpret_cast<double *>(sL + (size_t)k * 512 * PPL + 512 * u) *= rho[u];  // C_k
-    }
-    stage_wait();
-    __syncthreads();
-
-    double om[MAXOWN][PPL];
-#pragma unroll
-    for (int s = 0; s < MAXOWN; ++s)
-#pragma unroll
-        for (int u = 0; u < PPL; ++u) om[s][u] = 0.0;
-
-    const int nch = rs.n_chunks;
-    for (int ci = 0; ci < nch; ++ci) {
-        const int4 ch = sChunk[ci];
-        const char *blk = sStage + (size_t)(ci & 1) * rs.stage_bytes;
-        if (ci + 1 < nch)
-            stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, rs.stage + sChunk[ci + 1].z,
-                        rs.stage_bytes, threadIdx.x, 32 * W);
-        else  // behind the last chunk: the h/(RT) sets for the epilogue
-            stage_async(sStage + (size_t)((ci + 1) & 1) * rs.stage_bytes, reinterpret_cast<const unsigned char *>(rs.hco),
-                        128 * Ns, threadIdx.x, 32 * W);
-        const int count = ch.y;
-        constexpr int SLOT_ROW = 16 + 4 * MAXOWN;
-        const int o_slot = 48 * count, o_troe = o_slot + SLOT_ROW * W;
-        switch (ch.x) {
-        case 0: reaction_stage<W, PPL, 0, false>(blk, count, o_troe, sL, sQl, warp, c); break;
-        case 1: reaction_stage<W, PPL, 1, false>(blk, count, o_troe, sL, sQl, warp, c); break;
-        case 2: reaction_stage<W, PPL, 2, false>(blk, count, o_troe, sL, sQl, warp, c); break;
-        default: reaction_stage<W, PPL, 0, true>(blk, count, o_troe, sL, sQl, warp, c); break;
-        }
-        __syncthreads();
-        {
-            // the warp's entries are contiguous (slot-major); slot s ends at ends[s]; one entry is read ahead
-            const char *sr = blk + o_slot + SLOT_ROW * warp;
-            unsigned e = *reinterpret_cast<const unsigned *>(sr);
-            uint4 en0 = ldsu4(blk + e), en1 = ldsu4(blk + e + 16);
-#pragma unroll
-            for (int s4 = 0; s4 < MAXOWN; s4 += 4) {
-                const uint4 ends = ldsu4(sr + 16 + 4 * s4);
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int s = s4 + j;
-                    const unsigned end = j == 0 ? ends.x : (j == 1 ? ends.y : (j == 2 ? ends.z : ends.w));
-#pragma unroll 1
-                    while (e < end) {  // two entries per trip (lists are padded to even length)
-                        const uint4 c0 = en0, c1 = en1;
-                        e += 32;
-                        en0 = ldsu4(blk + e), en1 = ldsu4(blk + e + 16);
-                        const double nu0 = __hiloint2double((int)c0.y, (int)c0.x);
-                        const double nu1 = __hiloint2double((int)c1.y, (int)c1.x);
-                        double q0[PPL], q1[PPL];
-#pragma unroll
-                        for (int u = 0; u < PPL; ++u) {
-                            q0[u] = *reinterpret_cast<const double *>(sQl + c0.z + 256 * u);
-                            q1[u] = *reinterpret_cast<const double *>(sQl + c1.z + 256 * u);
-                        }
-#pragma unroll
-                        for (int u = 0; u < PPL; ++u) om[s][u] = fma(nu1, q1[u], fma(nu0, q0[u], om[s][u]));
-                    }
-                }
-            }
-        }
-        stage_wait();
-        __syncthreads();
-    }
-
-    // ---- store omega; a9: qdot = -sum_k h_k omega_k
-    double qd[PPL];
-#pragma unroll
-    for (int u = 0; u < PPL; ++u) qd[u] = 0.0;
-#pragma unroll
-    for (int s = 0; s < MAXOWN; ++s) {
-        const int k = warp + W * s;
-        if (k < Ns) {
-            const double2 *h = reinterpret_cast<const double2 *>(sStage + (size_t)(nch & 1) * rs.stage_bytes) + 8 * k;
-            const double2 l01 = h[0], l23 = h[1], l45 = h[2], l6t = h[3];
-            const double2 h01 = h[4], h23 = h[5], h45 = h[6];
-#pragma unroll
-            for (int u = 0; u < PPL; ++u) {
-                const double Tu = c.T[u];
-                double lo = fma(Tu, l45.x, l23.y);
-                lo = fma(Tu, lo, l23.x);
-                lo = fma(Tu, lo, l01.y);
-                lo = fma(Tu, lo, l01.x);
-                lo = fma(l45.y, c.rT[u], lo);
-                double hi = fma(Tu, h45.x, h23.y);
-                hi = fma(Tu, hi, h23.x);
-                hi = fma(Tu, hi, h01.y);
-                hi = fma(Tu, hi, h01.x);
-                hi = fma(h45.y, c.rT[u], hi);
-                qd[u] = fma(-(Tu <= l6t.y ? lo : hi), om[s][u], qd[u]);
-            }
-            store_row<PPL>(omega + (int64_t)k * n, i0, n, vec, om[s]);
-        }
-    }
-#pragma unroll
-    for (int u = 0; u < PPL; ++u) sred[(warp * PPL + u) * 32 + lane] = qd[u];
-    __syncthreads();
-    if (warp == 0) {
-        double out[PPL];
-#pragma unroll
-        for (int u = 0; u < PPL; ++u) {
-            double s = 0.0;
-#pragma unroll
-            for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
-            out[u] = s * (CRF_R_GAS * c.T[u]);
-        }
-        store_row<PPL>(qdot, i0, n, vec, out);
-    }
-}
-
-template <int W, int PPL, int MAXOWN>
-cudaError_t launch_k(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
-                     double *qdot, cudaStream_t st)
-{
-    const size_t smem = rates_smem_dynamic_smem(m);
-    cudaError_t e = cudaFuncSetAttribute(rates_smem_kernel<W, PPL, MAXOWN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)smem);
-    if (e != cudaSuccess) return e;
-    const int64_t per_block = 32 * PPL;
-    rates_smem_kernel<W, PPL, MAXOWN><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, p, Y, n,
-                                                                                                        omega, qdot);
-    crf_count_launch();
-    return cudaGetLastError();
-}
-
-template <int W, int PPL>
-cudaError_t launch_wp(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
-                      double *qdot, cudaStream_t st)
-{
-    const int own = (m.Ns + W - 1) / W;
-    if (own <= 4) return launch_k<W, PPL, 4>(m, T, p, Y, n, omega, qdot, st);
-    if (own <= 8) return launch_k<W, PPL, 8>(m, T, p, Y, n, omega, qdot, st);
-    if (own <= 16) return launch_k<W, PPL, 16>(m, T, p, Y, n, omega, qdot, st);
-    return cudaErrorInvalidValue;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -609,23 +305,13 @@ cudaError_t launch_thread(const DevTables &m, const double *T, const double *p, 
 
 size_t rates_smem_dynamic_smem(const DevTables &m)
 {
-    if (m.rs.W == 1)  // thread kernel: state + omega columns, all chunk blocks, g and h sets
-        return (size_t)(m.Ns + 1) * (2048 + 1024) + (size_t)m.rs.stage_bytes + 256 * (size_t)m.Ns;
-    return (size_t)(m.Ns + 1) * 512 * m.rs.PPL + (size_t)m.rs.Rc * 256 * m.rs.PPL + 2 * (size_t)m.rs.stage_bytes;
+    // state + omega columns, all chunk blocks, g and h sets
+    return (size_t)(m.Ns + 1) * (2048 + 1024) + (size_t)m.rs.stage_bytes + 256 * (size_t)m.Ns;
 }
 
 cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                               double *omega, double *qdot, cudaStream_t st)
 {
-    const int key = m.rs.W * 10 + m.rs.PPL;
-    switch (key) {
-    case 14: return launch_thread(m, T, p, Y, n, omega, qdot, st);
-    case 41: return launch_wp<4, 1>(m, T, p, Y, n, omega, qdot, st);
-    case 42: return launch_wp<4, 2>(m, T, p, Y, n, omega, qdot, st);
-    case 81: return launch_wp<8, 1>(m, T, p, Y, n, omega, qdot, st);
-    case 82: return launch_wp<8, 2>(m, T, p, Y, n, omega, qdot, st);
-    case 161: return launch_wp<16, 1>(m, T, p, Y, n, omega, qdot, st);
-    case 162: return launch_wp<16, 2>(m, T, p, Y, n, omega, qdot, st);
-    default: return cudaErrorInvalidValue;
-    }
+    if (m.rs.W != 1 || m.rs.PPL != 4) return cudaErrorInvalidValue;
+    return launch_thread(m, T, p, Y, n, omega, qdot, st);
 }

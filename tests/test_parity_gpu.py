@@ -212,6 +212,9 @@ PLAN_OVERRIDES = [
     dict(rates_kernel="group", rates_W=8, rates_PPL=1),
     dict(rates_kernel="group", rates_W=4, rates_PPL=2, rates_Rc=32),   # many small chunks
     dict(rates_kernel="group", rates_W=16, rates_PPL=2),
+    dict(rates_kernel="group", rates_tmem=1),              # u rows in shared memory (the path of Ns > 127)
+    dict(rates_kernel="group", rates_tmem=2),              # u rows in tensor memory, required
+    dict(rates_kernel="group", rates_W=16, rates_PPL=1, rates_tmem=2),
     dict(rates_kernel="staged"),                           # log-space K_c kernel (the automatic fall-back)
     dict(rates_kernel="generic"),                          # one thread per point, libm
     dict(rates_kernel="thread"),                           # one thread per point, product form (default for Ns <= 12)
@@ -226,6 +229,8 @@ def _admits(name, opt):
         return False
     if opt.get("rates_kernel") == "group" and opt.get("rates_W") and (Ns + opt["rates_W"] - 1) // opt["rates_W"] > 16:
         return False
+    if opt.get("rates_kernel") == "group" and Ns <= 12 and not opt.get("rates_W"):
+        pass  # (the warp-group kernel also takes small mechanisms on request)
     if opt.get("transport_kernel") == "small" and Ns > 16:
         return False
     if opt.get("transport_kernel") == "tiled" and Ns < 17:
@@ -254,8 +259,10 @@ def test_plan_overrides(binding, oracle_mod, name, opt):
     om = oracle_mod.Oracle(desc)
     info = gm.plan_info()
     for k, v in opt.items():
-        if k not in ("rates_Rc", "transport_panel"):
+        if k not in ("rates_Rc", "transport_panel", "rates_tmem"):
             assert info[k] == v, (k, info)
+    if "rates_tmem" in opt:
+        assert (info["rates_tmem_cols"] > 0) == (opt["rates_tmem"] == 2), info
     n = SMALL_N[name] + 2
     st = wl.make_state(name, n=n, total=n)
     parity.assert_parity(parity.run_gpu(gm, st), parity.run_oracle(om, st), f"{name} {opt} n={n}")
