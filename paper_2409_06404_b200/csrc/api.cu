@@ -100,6 +100,14 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
             g[5 * Ns] = a6, g[6 * Ns] = -a7;
         }
     }
+    std::vector<double> thermo_tab(14 * (size_t)Ns, 0.0);
+    for (int k = 0; k < Ns; ++k) {
+        for (int c = 0; c < 6; ++c) {
+            thermo_tab[14 * (size_t)k + c] = t->nasa_lo[(size_t)c * Ns + k] / W[k];
+            thermo_tab[14 * (size_t)k + 6 + c] = t->nasa_hi[(size_t)c * Ns + k] / W[k];
+        }
+        thermo_tab[14 * (size_t)k + 12] = Tmid[k];
+    }
     std::vector<double> lnA(t->lnA, t->lnA + Nr), beta(t->beta, t->beta + Nr), Ea_R(t->Ea_R, t->Ea_R + Nr), dnu(Nr);
     std::vector<int16_t> reac(t->reac, t->reac + (size_t)kSlots * Nr), prod(t->prod, t->prod + (size_t)kSlots * Nr);
     for (int r = 0; r < Nr; ++r) {
@@ -160,7 +168,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
                  oreac = b.add(reac), oprod = b.add(prod), oep = b.add(eff_ptr), oei = b.add(eff_idx),
                  oev = b.add(eff_val), olnA0 = b.add(lnA0), ob0 = b.add(beta0), oE0 = b.add(Ea0_R), oal = b.add(alpha),
                  orT3 = b.add(rT3), orT1 = b.add(rT1), oT2 = b.add(T2), omu = b.add(mu_c), olam = b.add(lam_c),
-                 onD = b.add(nDc), owk = b.add(wilke), owq = b.add(wq);
+                 onD = b.add(nDc), owk = b.add(wilke), owq = b.add(wq), otht = b.add(thermo_tab);
     const TransportPlanOffsets tpo = build_transport_plan(t, opt, b);
     const RatesPlanOffsets rpo = build_rates_plan(t, opt, b);
     const RatesSmemPlanOffsets rso = build_rates_smem_plan(t, opt, b);
@@ -211,6 +219,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
     d.eff_val = D(oev);
     d.lnA0 = D(olnA0), d.beta0 = D(ob0), d.Ea0_R = D(oE0), d.alpha = D(oal), d.rT3 = D(orT3), d.rT1 = D(orT1),
     d.T2 = D(oT2);
+    d.thermo_tab = D(otht);
     d.mu_c = D(omu), d.lam_c = D(olam), d.nDc = D(onD), d.wilke_c = D(owk), d.wq = D(owq);
     TransportPlan &tp = d.tp;
     tp.W = tpo.W, tp.PPL = tpo.PPL, tp.NsP = tpo.NsP, tp.nb = tpo.nb, tp.n_wilke = tpo.n_wilke, tp.n_rounds = tpo.n_rounds;

@@ -132,6 +132,8 @@ struct DevTables {
     //   gc[7]:  g/(RT) = c0 (1 - ln T) + T (c1 + T (c2 + T (c3 + T c4))) + c5/T + c6
     //                    (c1..c4 = -a2/2, -a3/6, -a4/12, -a5/20; c5 = a6; c6 = -a7)
     const double *cpc, *hc, *gc, *sc;  // sc[6]: s/R = c0 ln T + T(c1 + ...c4) + c5
+    // crf_thermo (thermo.cu): [Ns][14] = {a1..a5, a6} / W_k of the low range, of the high range, then T_mid, pad
+    const double *thermo_tab;
     // reactions (sorted elementary | third-body | falloff)
     const double *lnA, *beta, *Ea_R, *dnu;  // [Nr]; dnu = sum nu'' - sum nu'
     const int16_t *reac, *prod;             // [3][Nr]

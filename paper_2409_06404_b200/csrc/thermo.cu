@@ -1,63 +1,119 @@
 // thermo.cu -- crf_thermo / crf_thermo_species kernels.
 //
-// HBM-bound streaming kernels: one thread per grid point, Y[k*n + i] read once with
-// coalesced loads (a warp reads 256 contiguous bytes per species), NASA-7 coefficients
-// staged once per block into shared memory in the Horner forms of crf_internal.h.
-// The per-lane range select (T <= Tmid_k) is a shared-memory address select, not a branch.
+// crf_thermo is an HBM stream: Y[k*n + i] is read once, 8 (Ns + 1) + 16 bytes per point.  To stay under the stream's
+// time on the FP64 pipe the mixture sums are accumulated as MOMENTS of the NASA-7 coefficients,
+//     M_c = sum_k (Y_k / W_k) a_{c+1,k}(range of T),  c = 0..4,   M_5 = sum_k (Y_k / W_k) a_{6,k}
+//     c_p = R (M_0 + T (M_1 + T (M_2 + T (M_3 + T M_4))))
+//     h   = R T (M_0 + T (M_1/2 + T (M_2/3 + T (M_3/4 + T M_4/5))) + M_5/T)
+// six FMAs per species and point instead of the thirteen of two Horner evaluations (c_p and h share their
+// coefficients).  The table (a_c/W_k: the six of the low range, then the six of the high range, so that a lane's range
+// select is an address offset of 48 bytes and a set is three 128-bit loads) is staged once
+// per block into shared memory; a thread owns two adjacent points (128-bit loads of the Y rows), the species loop
+// is unrolled by four so that four row loads are in flight per thread, and a block walks several point groups.
+// The range select T <= T_mid compares the bit patterns as integers (both are positive): no FP64 pipe instruction.
 #include "crf_internal.h"
+#include <algorithm>
+
 #include "launch.h"
 
 namespace {
 
 constexpr int TB = 256;
+constexpr int TH_MINB = 3;    // blocks per SM (80 registers: no spills; measured against 2 and 4)
+constexpr int TH_UNROLL = 4;  // species rows in flight per thread
+constexpr int TH_STRIDE = 14;  // doubles per species in the table: 6 low-range, 6 high-range coefficients, T_mid, pad
 
-// smem: [2][11][Ns] = cpc(5) then hc(6) per range
-__global__ void __launch_bounds__(TB) thermo_kernel(DevTables m, const double *__restrict__ T,
-                                                    const double *__restrict__ Y, int64_t n,
-                                                    double *__restrict__ cp, double *__restrict__ h)
+template <int P>
+__device__ __forceinline__ void thermo_species_step(const double *__restrict__ tab, int k, const double (&y)[P],
+                                                    const long long (&Tbits)[P], double (&M)[6][P])
 {
-    extern __shared__ double sm[];
+    const double *row = tab + TH_STRIDE * k;
+    const long long tmid = __double_as_longlong(row[12]);
+#pragma unroll
+    for (int u = 0; u < P; ++u) {
+        const double2 *c = reinterpret_cast<const double2 *>(row + (Tbits[u] <= tmid ? 0 : 6));
+        const double2 c01 = c[0], c23 = c[1], c45 = c[2];
+        M[0][u] = fma(y[u], c01.x, M[0][u]), M[1][u] = fma(y[u], c01.y, M[1][u]);
+        M[2][u] = fma(y[u], c23.x, M[2][u]), M[3][u] = fma(y[u], c23.y, M[3][u]);
+        M[4][u] = fma(y[u], c45.x, M[4][u]), M[5][u] = fma(y[u], c45.y, M[5][u]);
+    }
+}
+
+template <int P>
+__device__ __forceinline__ void thermo_finish(const double (&M)[6][P], const double (&Ti)[P], double (&cp)[P], double (&h)[P])
+{
+#pragma unroll
+    for (int u = 0; u < P; ++u) {
+        const double T = Ti[u];
+        double c = fma(T, M[4][u], M[3][u]);
+        c = fma(T, c, M[2][u]);
+        c = fma(T, c, M[1][u]);
+        c = fma(T, c, M[0][u]);
+        cp[u] = c * CRF_R_GAS;
+        double e = fma(T, M[4][u] * 0.2, M[3][u] * 0.25);
+        e = fma(T, e, M[2][u] * (1.0 / 3.0));
+        e = fma(T, e, M[1][u] * 0.5);
+        e = fma(T, e, M[0][u]);
+        h[u] = fma(T, e, M[5][u]) * CRF_R_GAS;  // R T (e + M_5 / T)
+    }
+}
+
+__global__ void __launch_bounds__(TB, TH_MINB) thermo_kernel(DevTables m, const double *__restrict__ T,
+                                                       const double *__restrict__ Y, int64_t n,
+                                                       double *__restrict__ cp, double *__restrict__ h)
+{
+    extern __shared__ __align__(16) double sm[];
     const int Ns = m.Ns;
-    double *s_tmid = sm;            // [Ns]
-    double *s_rW = sm + Ns;         // [Ns]
-    double *s_co = sm + 2 * Ns;     // [2][11][Ns]
-    for (int idx = threadIdx.x; idx < Ns; idx += TB) {
-        s_tmid[idx] = m.Tmid[idx];
-        s_rW[idx] = m.rW[idx];
-    }
-    for (int idx = threadIdx.x; idx < 2 * 5 * Ns; idx += TB) {
-        int rg = idx / (5 * Ns), rem = idx % (5 * Ns);
-        s_co[rg * 11 * Ns + rem] = m.cpc[idx];
-    }
-    for (int idx = threadIdx.x; idx < 2 * 6 * Ns; idx += TB) {
-        int rg = idx / (6 * Ns), rem = idx % (6 * Ns);
-        s_co[rg * 11 * Ns + 5 * Ns + rem] = m.hc[idx];
-    }
+    for (int idx = threadIdx.x; idx < TH_STRIDE * Ns; idx += TB) sm[idx] = __ldg(m.thermo_tab + idx);
     __syncthreads();
-    const int64_t i = (int64_t)blockIdx.x * TB + threadIdx.x;
-    if (i >= n) return;
-    const double Ti = T[i];
-    const double rT = 1.0 / Ti;
-    double cpm = 0.0, hm = 0.0;
-#pragma unroll 2
-    for (int k = 0; k < Ns; ++k) {
-        const double y = Y[(int64_t)k * n + i] * s_rW[k];
-        const double *c = s_co + ((Ti <= s_tmid[k]) ? 0 : 11 * Ns) + k;
-        double cpk = fma(Ti, c[4 * Ns], c[3 * Ns]);
-        cpk = fma(Ti, cpk, c[2 * Ns]);
-        cpk = fma(Ti, cpk, c[1 * Ns]);
-        cpk = fma(Ti, cpk, c[0]);
-        const double *d = c + 5 * Ns;
-        double hk = fma(Ti, d[4 * Ns], d[3 * Ns]);
-        hk = fma(Ti, hk, d[2 * Ns]);
-        hk = fma(Ti, hk, d[1 * Ns]);
-        hk = fma(Ti, hk, d[0]);
-        hk = fma(d[5 * Ns], rT, hk);
-        cpm = fma(y, cpk, cpm);
-        hm = fma(y, hk, hm);
+    const bool vec = (n & 1) == 0;
+    const int64_t npair = (n + 1) >> 1;
+    for (int64_t j = (int64_t)blockIdx.x * TB + threadIdx.x; j < npair; j += (int64_t)gridDim.x * TB) {
+        const int64_t i = 2 * j;
+        if (vec) {
+            const double2 t2 = *reinterpret_cast<const double2 *>(T + i);
+            const double Ti[2] = {t2.x, t2.y};
+            const long long Tb[2] = {__double_as_longlong(t2.x), __double_as_longlong(t2.y)};
+            double M[6][2];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) M[c][0] = M[c][1] = 0.0;
+            int k = 0;
+            for (; k + TH_UNROLL <= Ns; k += TH_UNROLL) {
+                double2 y4[TH_UNROLL];
+#pragma unroll
+                for (int q = 0; q < TH_UNROLL; ++q) y4[q] = *reinterpret_cast<const double2 *>(Y + (int64_t)(k + q) * n + i);
+#pragma unroll
+                for (int q = 0; q < TH_UNROLL; ++q) {
+                    const double y[2] = {y4[q].x, y4[q].y};
+                    thermo_species_step<2>(sm, k + q, y, Tb, M);
+                }
+            }
+            for (; k < Ns; ++k) {
+                const double2 yy = *reinterpret_cast<const double2 *>(Y + (int64_t)k * n + i);
+                const double y[2] = {yy.x, yy.y};
+                thermo_species_step<2>(sm, k, y, Tb, M);
+            }
+            double c2[2], h2[2];
+            thermo_finish<2>(M, Ti, c2, h2);
+            *reinterpret_cast<double2 *>(cp + i) = make_double2(c2[0], c2[1]);
+            *reinterpret_cast<double2 *>(h + i) = make_double2(h2[0], h2[1]);
+        } else {
+            for (int64_t ii = i; ii < n && ii < i + 2; ++ii) {  // odd n: rows are not 16-byte aligned, scalar accesses
+                const double Ti[1] = {T[ii]};
+                const long long Tb[1] = {__double_as_longlong(Ti[0])};
+                double M[6][1];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) M[c][0] = 0.0;
+                for (int k = 0; k < Ns; ++k) {
+                    const double y[1] = {Y[(int64_t)k * n + ii]};
+                    thermo_species_step<1>(sm, k, y, Tb, M);
+                }
+                double c1[1], h1[1];
+                thermo_finish<1>(M, Ti, c1, h1);
+                cp[ii] = c1[0], h[ii] = h1[0];
+            }
+        }
     }
-    cp[i] = cpm * CRF_R_GAS;
-    h[i] = hm * (CRF_R_GAS * Ti);
 }
 
 __global__ void __launch_bounds__(TB) thermo_species_kernel(DevTables m, const double *__restrict__ T, int64_t n,
@@ -99,13 +155,10 @@ __global__ void __launch_bounds__(TB) thermo_species_kernel(DevTables m, const d
 cudaError_t launch_thermo(const DevTables &m, const double *T, const double *Y, int64_t n, double *cp, double *h,
                           cudaStream_t st)
 {
-    const size_t smem = sizeof(double) * (size_t)(2 + 22) * m.Ns;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaFuncSetAttribute(thermo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        attr_done = true;
-    }
-    const int64_t blocks = (n + TB - 1) / TB;
+    const size_t smem = sizeof(double) * TH_STRIDE * (size_t)m.Ns;
+    const int64_t npair = (n + 1) / 2;
+    // TH_MINB blocks of 8 warps per SM; a block walks its share of the point pairs (the table is staged once per block)
+    const int64_t blocks = std::min<int64_t>((npair + TB - 1) / TB, 148 * TH_MINB * 4);
     thermo_kernel<<<(unsigned)blocks, TB, smem, st>>>(m, T, Y, n, cp, h);
     crf_count_launch();
     return cudaGetLastError();
