@@ -323,3 +323,27 @@ void oracle_mix_transport(const oracle_mech *m, const double *T, const double *p
         free(buf);
     }
 }
+
+/* ---- everything one evaluation of the right-hand side consumes at a grid point ------------------
+ * "The right-hand side (RHS) function, evaluated in each Newton step and linear iteration, employs ... kernels for
+ * ... species production rates, and thermodynamic and transport properties": omega_k and the heat
+ * release of Eq. 1a-1b, c_p and c_{p,k} of Eq. 1b-1c, rho of Eq. 1d, the mean molar
+ * mass Wbar, lambda (Eq. 1b), D_k (Eq. 2) and mu (Eq. 4).
+ * A plain composition of the functions above (no shared intermediates) plus
+ *   Wbar = 1 / sum_k Y_k / W_k [kg/kmol],   rho = p Wbar / (R T) [kg/m^3],   cpk = molar c_{p,k} [J/(kmol K)]. */
+void oracle_rhs_pointwise(const oracle_mech *m, const double *T, const double *p, const double *Y, int64_t n,
+                          double *omega, double *qdot, double *S_omega, double *S_q,
+                          double *cp, double *h, double *h_scale, double *cpk, double *rho, double *Wbar,
+                          double *mu, double *lambda, double *rhoD)
+{
+    oracle_production_rates(m, T, p, Y, n, omega, qdot, S_omega, S_q);
+    oracle_thermo(m, T, p, Y, n, cp, h, h_scale);
+    oracle_thermo_species(m, T, n, cpk, 0, 0, 0);
+    oracle_mix_transport(m, T, p, Y, n, mu, lambda, rhoD, 0);
+    for (int64_t i = 0; i < n; ++i) {
+        double inv_W = 0.0;
+        for (int k = 0; k < m->Ns; ++k) inv_W += Y[k * n + i] / m->W[k];
+        Wbar[i] = 1.0 / inv_W;
+        rho[i] = p[i] * Wbar[i] / (R_GAS * T[i]);
+    }
+}

@@ -153,3 +153,35 @@ class Oracle:
         _lib.oracle_mix_transport(C.byref(self._m), _ptr(T), _ptr(p), _ptr(Y), C.c_int64(n),
                                   _ptr(mu), _ptr(lam), _ptr(rhoD), _ptr(Dkm))
         return dict(mu=mu, lam=lam, rhoD=rhoD, Dkm=Dkm)
+
+    def rhs_pointwise(self, T, p, Y):
+        """dict of everything one right-hand-side evaluation consumes (oracle_rhs_pointwise):
+        omega, qdot, S_omega, S_q, cp, h, h_scale, cpk [Ns,n] J/kmol/K, rho [n] kg/m^3, Wbar [n] kg/kmol, mu, lam, rhoD."""
+        T, p, Y, n = self._state(T, p, Y)
+        o = {k: np.empty((self.Ns, n)) for k in ("omega", "S_omega", "cpk", "rhoD")}
+        o.update({k: np.empty(n) for k in ("qdot", "S_q", "cp", "h", "h_scale", "rho", "Wbar", "mu", "lam")})
+        order = ("omega", "qdot", "S_omega", "S_q", "cp", "h", "h_scale", "cpk", "rho", "Wbar", "mu", "lam", "rhoD")
+        _lib.oracle_rhs_pointwise(C.byref(self._m), _ptr(T), _ptr(p), _ptr(Y), C.c_int64(n), *[_ptr(o[k]) for k in order])
+        return o
+
+    def production_rates_pair(self, T, p, Y, T2, p2, Y2):
+        """omega and qdot at two states of the same points: two plain calls."""
+        a, b = self.production_rates(T, p, Y), self.production_rates(T2, p2, Y2)
+        return dict(omega=a["omega"], qdot=a["qdot"], S_omega=a["S_omega"], S_q=a["S_q"],
+                    omega2=b["omega"], qdot2=b["qdot"], S_omega2=b["S_omega"], S_q2=b["S_q"])
+
+    def production_rates_jv(self, T, p, Y, dT, dp, dY, sigma):
+        """the difference quotient behind the matrix-free Jacobian-vector product:
+        J v ~ (omega(y + sigma v) - omega(y)) / sigma with y = (T, p, Y), v = (dT, dp, dY).  The perturbed state is
+        formed in double with one rounding per operation (multiply, then add); then two plain calls and the quotient.
+        The tolerance scale of the quotient is (S(y) + S(y + sigma v)) / sigma."""
+        T, p, Y, n = self._state(T, p, Y)
+        dT, dp, dY, _ = self._state(dT, dp, dY)
+        sigma = float(sigma)
+        T2, p2, Y2 = T + sigma * dT, p + sigma * dp, Y + sigma * dY
+        r = self.production_rates_pair(T, p, Y, T2, p2, Y2)
+        r["Jomega"] = (r["omega2"] - r["omega"]) / sigma
+        r["Jqdot"] = (r["qdot2"] - r["qdot"]) / sigma
+        r["S_Jomega"] = (r["S_omega"] + r["S_omega2"]) / abs(sigma)
+        r["S_Jqdot"] = (r["S_q"] + r["S_q2"]) / abs(sigma)
+        return r
