@@ -142,6 +142,41 @@ int crf_production_rates(const crf_mech *mech, const double *T, const double *p,
 int crf_mix_transport(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
                       double *mu, double *lambda, double *rhoD);
 
+/* Everything one evaluation of the right-hand side consumes at a grid point, in one call.  "The
+ * right-hand side (RHS) function, evaluated in each Newton step and linear iteration, employs ... kernels for ...
+ * species production rates, and thermodynamic and transport properties": omega_k and the heat release
+ * of Eq. 1a-1b, c_p and c_{p,k} of Eq. 1b-1c, rho of Eq. 1d, the
+ * mean molar mass, lambda, D_k (Eq. 2) and mu (Eq. 4).  The outputs shared
+ * with crf_thermo, crf_production_rates and crf_mix_transport are defined as there; in addition
+ *   cpk[Ns*n]  molar c_{p,k}, species-major              [J/(kmol K)]   (may be NULL)
+ *   rho[n]     p Wbar / (R T)                            [kg/m^3]
+ *   Wbar[n]    1 / sum_k Y_k / W_k                       [kg/kmol]
+ * The thermodynamic outputs are by-products of the production-rates kernel (no separate pass over Y); transport is
+ * a second kernel on the same stream.  Mechanisms without a warp-group rates plan take the separate kernels. */
+int crf_rhs_pointwise(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *omega,
+                      double *qdot, double *cp, double *h, double *cpk, double *rho, double *Wbar, double *mu,
+                      double *lambda, double *rhoD);
+
+/* Production rates at TWO states of the same n points in one launch: the matrix-free Newton-Krylov
+ * solver of the paper approximates Jacobian-vector products by difference quotients, so the rates
+ * are wanted at y and at a perturbed y' = y + sigma v.  Both states of a point share a lane of the kernel: mechanism
+ * tables, reaction records and incidence lists are read once for the two evaluations.  Results are bit-identical to
+ * two crf_production_rates calls whenever both run the same kernel.  (T2, p2, Y2) -> (omega2, qdot2). */
+int crf_production_rates_pair(const crf_mech *mech, const double *T, const double *p, const double *Y, const double *T2,
+                              const double *p2, const double *Y2, int64_t n, double *omega, double *qdot, double *omega2,
+                              double *qdot2);
+
+/* The difference quotient itself: the perturbed state y' = (T + sigma dT, p + sigma dp, Y + sigma dY) is formed in
+ * the kernel (multiply, then add: one rounding each, as a host would), both states are evaluated in one launch and
+ *   Jomega[Ns*n] = (omega(y') - omega(y)) / sigma,   Jqdot[n] = (qdot(y') - qdot(y)) / sigma
+ * are returned next to omega(y), qdot(y) (omega and qdot may both be NULL).  dp may be NULL (no pressure
+ * perturbation).  sigma must be finite and non-zero.  Each value of the quotient carries the rounding of two
+ * evaluations divided by sigma: its tolerance scale is (S(y) + S(y')) / |sigma|.  CRF_EUNSUPPORTED for a mechanism
+ * whose plan cannot hold two states per lane (explicit one-point-per-lane or fall-back kernels). */
+int crf_production_rates_jv(const crf_mech *mech, const double *T, const double *p, const double *Y, const double *dT,
+                            const double *dp, const double *dY, double sigma, int64_t n, double *omega, double *qdot,
+                            double *Jomega, double *Jqdot);
+
 /* One pass of the whole path with HOST buffers: copies T, p, Y to the device in chunks, runs
  * crf_thermo, crf_production_rates and crf_mix_transport on each chunk and copies the seven
  * outputs back, chunks pipelined over internal streams.  All pointers are host pointers with

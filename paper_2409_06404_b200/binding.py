@@ -19,7 +19,8 @@ _lib = None
 # include/crf.h (the method) and include/crf_diag.h (plan control, diagnostics)
 EXPORTS = ("crf_mech_create", "crf_mech_destroy", "crf_mech_set_stream", "crf_mech_num_species",
            "crf_mech_num_reactions", "crf_thermo", "crf_thermo_species", "crf_production_rates",
-           "crf_mix_transport", "crf_step_host", "crf_last_error")
+           "crf_mix_transport", "crf_rhs_pointwise", "crf_production_rates_pair", "crf_production_rates_jv",
+           "crf_step_host", "crf_last_error")
 EXPORTS_DIAG = ("crf_mech_create_ex", "crf_mech_plan_info", "crf_fp64_probe", "crf_launch_count",
                 "crf_transport_schedule")
 
@@ -68,6 +69,9 @@ def lib() -> C.CDLL:
         L.crf_thermo_species.argtypes = [vp, dp, i64, dp, dp, dp]
         L.crf_production_rates.argtypes = [vp, dp, dp, dp, i64, dp, dp]
         L.crf_mix_transport.argtypes = [vp, dp, dp, dp, i64, dp, dp, dp]
+        L.crf_rhs_pointwise.argtypes = [vp, dp, dp, dp, i64] + [dp] * 10
+        L.crf_production_rates_pair.argtypes = [vp] + [dp] * 6 + [i64] + [dp] * 4
+        L.crf_production_rates_jv.argtypes = [vp] + [dp] * 6 + [C.c_double, i64] + [dp] * 4
         L.crf_step_host.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
         L.crf_fp64_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.crf_launch_count.restype = C.c_int64
@@ -182,6 +186,46 @@ class Mechanism:
         _check(lib().crf_mix_transport(self._h, _dev(T, (n,)), _dev(p), _dev(Y, (self.Ns, n)), n,
                                        _dev(mu, (n,)), _dev(lam, (n,)), _dev(rhoD, (self.Ns, n))))
         return mu, lam, rhoD
+
+    def rhs_pointwise(self, T, p, Y, out: dict | None = None, want_cpk: bool = True) -> dict:
+        """``crf_rhs_pointwise``: dict(omega, qdot, cp, h, cpk, rho, Wbar, mu, lam, rhoD) of device tensors."""
+        n = T.numel()
+        if out is None:
+            out = {k: torch.empty_like(T) for k in ("qdot", "cp", "h", "rho", "Wbar", "mu", "lam")}
+            out.update({k: torch.empty_like(Y) for k in ("omega", "rhoD")})
+            out["cpk"] = torch.empty_like(Y) if want_cpk else None
+        self._sync_stream()
+        _check(lib().crf_rhs_pointwise(
+            self._h, _dev(T, (n,)), _dev(p, (n,)), _dev(Y, (self.Ns, n)), n, _dev(out["omega"], (self.Ns, n)),
+            _dev(out["qdot"], (n,)), _dev(out["cp"], (n,)), _dev(out["h"], (n,)), _dev(out.get("cpk")),
+            _dev(out["rho"], (n,)), _dev(out["Wbar"], (n,)), _dev(out["mu"], (n,)), _dev(out["lam"], (n,)),
+            _dev(out["rhoD"], (self.Ns, n))))
+        return out
+
+    def production_rates_pair(self, T, p, Y, T2, p2, Y2, out=None):
+        """``crf_production_rates_pair``: (omega, qdot, omega2, qdot2)."""
+        n = T.numel()
+        if out is None:
+            out = (torch.empty_like(Y), torch.empty_like(T), torch.empty_like(Y), torch.empty_like(T))
+        self._sync_stream()
+        _check(lib().crf_production_rates_pair(
+            self._h, _dev(T, (n,)), _dev(p, (n,)), _dev(Y, (self.Ns, n)), _dev(T2, (n,)), _dev(p2, (n,)),
+            _dev(Y2, (self.Ns, n)), n, _dev(out[0], (self.Ns, n)), _dev(out[1], (n,)), _dev(out[2], (self.Ns, n)),
+            _dev(out[3], (n,))))
+        return out
+
+    def production_rates_jv(self, T, p, Y, dT, dp, dY, sigma, out=None, base=True):
+        """``crf_production_rates_jv``: (omega, qdot, Jomega, Jqdot); omega, qdot are None when ``base`` is False."""
+        n = T.numel()
+        if out is None:
+            out = (torch.empty_like(Y) if base else None, torch.empty_like(T) if base else None,
+                   torch.empty_like(Y), torch.empty_like(T))
+        self._sync_stream()
+        _check(lib().crf_production_rates_jv(
+            self._h, _dev(T, (n,)), _dev(p, (n,)), _dev(Y, (self.Ns, n)), _dev(dT, (n,)), _dev(dp),
+            _dev(dY, (self.Ns, n)), float(sigma), n, _dev(out[0]), _dev(out[1]), _dev(out[2], (self.Ns, n)),
+            _dev(out[3], (n,))))
+        return out
 
     def step_host(self, T, p, Y, out: dict | None = None) -> dict:
         """Whole path with HOST tensors (pinned for full bandwidth); returns host tensors."""

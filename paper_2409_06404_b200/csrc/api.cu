@@ -172,7 +172,9 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
     const TransportPlanOffsets tpo = build_transport_plan(t, opt, b);
     const RatesPlanOffsets rpo = build_rates_plan(t, opt, b);
     const RatesSmemPlanOffsets rso = build_rates_smem_plan(t, opt, b);
-    const RatesGroupPlanOffsets rgo = rso.W > 0 ? RatesGroupPlanOffsets() : build_rates_group_plan(t, opt, b);
+    // (small mechanisms run the thread kernel for crf_production_rates; the warp-group plan is still built: it serves the
+    // pair / difference-quotient / fused right-hand-side calls, which evaluate two states or emit by-products per launch)
+    const RatesGroupPlanOffsets rgo = build_rates_group_plan(t, opt, b);
     // what will run, and whether that is what was asked for
     crf_plan_info info{};
     info.rates_kernel = rso.W > 0 ? CRF_RATES_THREAD
@@ -352,6 +354,79 @@ int crf_mix_transport(const crf_mech *mech, const double *T, const double *p, co
         return fail(CRF_EINVAL, "crf_mix_transport: pointers must be 16-byte aligned");
     cudaError_t e = launch_transport(mech->dev, T, p, Y, n, mu, lambda, rhoD, mech->stream);
     return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_mix_transport");
+}
+
+int crf_production_rates_pair(const crf_mech *mech, const double *T, const double *p, const double *Y, const double *T2,
+                              const double *p2, const double *Y2, int64_t n, double *omega, double *qdot, double *omega2,
+                              double *qdot2)
+{
+    CRF_CHECK_COMMON("crf_production_rates_pair")
+    if (!T || !p || !Y || !T2 || !p2 || !Y2 || !omega || !qdot || !omega2 || !qdot2)
+        return fail(CRF_EINVAL, "crf_production_rates_pair: null pointer");
+    for (const void *q : {(const void *)T, (const void *)p, (const void *)Y, (const void *)T2, (const void *)p2,
+                          (const void *)Y2, (const void *)omega, (const void *)qdot, (const void *)omega2, (const void *)qdot2})
+        if (misaligned(q)) return fail(CRF_EINVAL, "crf_production_rates_pair: pointers must be 16-byte aligned");
+    cudaError_t e;
+    if (mech->dev.rg.W > 0 && mech->dev.rg.PPL == 2) {
+        RatesIO io = rates_io(T, p, Y, omega, qdot);
+        io.T2 = T2, io.p2 = p2, io.Y2 = Y2, io.omega2 = omega2, io.qdot2 = qdot2, io.mode = 1;
+        e = launch_rates_group(mech->dev, io, n, mech->stream);
+    } else {  // no plan that shares a launch: two launches of whatever kernel the mechanism runs
+        e = launch_rates(mech->dev, T, p, Y, n, omega, qdot, mech->stream);
+        if (e == cudaSuccess) e = launch_rates(mech->dev, T2, p2, Y2, n, omega2, qdot2, mech->stream);
+    }
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_production_rates_pair");
+}
+
+int crf_production_rates_jv(const crf_mech *mech, const double *T, const double *p, const double *Y, const double *dT,
+                            const double *dp, const double *dY, double sigma, int64_t n, double *omega, double *qdot,
+                            double *Jomega, double *Jqdot)
+{
+    CRF_CHECK_COMMON("crf_production_rates_jv")
+    if (!T || !p || !Y || !dT || !dY || !Jomega || !Jqdot) return fail(CRF_EINVAL, "crf_production_rates_jv: null pointer");
+    if (!(sigma != 0.0) || !std::isfinite(sigma)) return fail(CRF_EINVAL, "crf_production_rates_jv: sigma must be finite and non-zero");
+    if ((omega == nullptr) != (qdot == nullptr))
+        return fail(CRF_EINVAL, "crf_production_rates_jv: omega and qdot must be given or omitted together");
+    for (const void *q : {(const void *)T, (const void *)p, (const void *)Y, (const void *)dT, (const void *)dp,
+                          (const void *)dY, (const void *)omega, (const void *)qdot, (const void *)Jomega, (const void *)Jqdot})
+        if (misaligned(q)) return fail(CRF_EINVAL, "crf_production_rates_jv: pointers must be 16-byte aligned");
+    if (!(mech->dev.rg.W > 0 && mech->dev.rg.PPL == 2))
+        return fail(CRF_EUNSUPPORTED, "crf_production_rates_jv: this mechanism has no warp-group plan with two states per lane "
+                                      "(use crf_production_rates_pair on a perturbed copy)");
+    RatesIO io = rates_io(T, p, Y, omega, qdot);
+    io.T2 = dT, io.p2 = dp, io.Y2 = dY, io.omega2 = Jomega, io.qdot2 = Jqdot, io.sigma = sigma, io.mode = 2;
+    cudaError_t e = launch_rates_group(mech->dev, io, n, mech->stream);
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_production_rates_jv");
+}
+
+int crf_rhs_pointwise(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *omega,
+                      double *qdot, double *cp, double *h, double *cpk, double *rho, double *Wbar, double *mu,
+                      double *lambda, double *rhoD)
+{
+    CRF_CHECK_COMMON("crf_rhs_pointwise")
+    if (!T || !p || !Y || !omega || !qdot || !cp || !h || !rho || !Wbar || !mu || !lambda || !rhoD)
+        return fail(CRF_EINVAL, "crf_rhs_pointwise: null pointer (only cpk may be omitted)");
+    for (const void *q : {(const void *)T, (const void *)p, (const void *)Y, (const void *)omega, (const void *)qdot,
+                          (const void *)cp, (const void *)h, (const void *)cpk, (const void *)rho, (const void *)Wbar,
+                          (const void *)mu, (const void *)lambda, (const void *)rhoD})
+        if (misaligned(q)) return fail(CRF_EINVAL, "crf_rhs_pointwise: pointers must be 16-byte aligned");
+    const DevTables &d = mech->dev;
+    cudaStream_t st = mech->stream;
+    cudaError_t e;
+    if (d.rg.W > 0) {
+        // the thermodynamic by-products leave the production-rates kernel (it evaluates the NASA sets and the
+        // composition anyway): no separate thermo pass, Y is read by two kernels instead of three
+        RatesIO io = rates_io(T, p, Y, omega, qdot);
+        io.cp = cp, io.h = h, io.cpk = cpk, io.rho = rho, io.Wbar = Wbar;
+        e = launch_rates_group(d, io, n, st);
+    } else {
+        e = launch_rates(d, T, p, Y, n, omega, qdot, st);
+        if (e == cudaSuccess) e = launch_thermo(d, T, Y, n, cp, h, st);
+        if (e == cudaSuccess && cpk) e = launch_thermo_species(d, T, n, cpk, nullptr, nullptr, st);
+        if (e == cudaSuccess) e = launch_density(d, T, p, Y, n, rho, Wbar, st);
+    }
+    if (e == cudaSuccess) e = launch_transport(d, T, p, Y, n, mu, lambda, rhoD, st);
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_rhs_pointwise");
 }
 
 // Chunked host pipeline: slot s owns a stream and one device buffer holding, for a chunk of c points,

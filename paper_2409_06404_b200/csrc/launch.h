@@ -4,10 +4,33 @@
 
 void crf_count_launch();
 
+// What one launch of the production-rates kernels reads and writes (device pointers).
+//   mode 0  omega, qdot at (T, p, Y); optionally the thermodynamic by-products of the same pass (crf_rhs_pointwise)
+//   mode 1  two states of the same points in one launch: (T, p, Y) -> omega, qdot and (T2, p2, Y2) -> omega2, qdot2
+//   mode 2  difference quotient: second state = (T, p, Y) + sigma (T2, p2, Y2) formed in the kernel (p2 may be null = 0);
+//           omega, qdot of the base state (may be null) and omega2, qdot2 = (f(second) - f(base)) / sigma
+struct RatesIO {
+    const double *T, *p, *Y;
+    const double *T2, *p2, *Y2;
+    double sigma;
+    int mode;
+    double *omega, *qdot;
+    double *omega2, *qdot2;
+    double *cp, *h, *cpk, *rho, *Wbar;  // mode 0 only, any may be null: mixture c_p, h; molar c_pk [Ns*n]; rho; Wbar
+};
+inline RatesIO rates_io(const double *T, const double *p, const double *Y, double *omega, double *qdot)
+{
+    RatesIO io{};
+    io.T = T, io.p = p, io.Y = Y, io.omega = omega, io.qdot = qdot;
+    return io;
+}
+
 cudaError_t launch_thermo(const DevTables &m, const double *T, const double *Y, int64_t n, double *cp, double *h,
                           cudaStream_t st);
 cudaError_t launch_thermo_species(const DevTables &m, const double *T, int64_t n, double *cpk, double *hk, double *sk,
                                   cudaStream_t st);
+cudaError_t launch_density(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *rho,
+                           double *Wbar, cudaStream_t st);
 cudaError_t launch_rates(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                          double *omega, double *qdot, cudaStream_t st);
 cudaError_t launch_transport(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
@@ -20,8 +43,7 @@ cudaError_t launch_rates_staged(const DevTables &m, const double *T, const doubl
                                 double *omega, double *qdot, cudaStream_t st);
 cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                               double *omega, double *qdot, cudaStream_t st);
-cudaError_t launch_rates_group(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
-                               double *omega, double *qdot, cudaStream_t st);
+cudaError_t launch_rates_group(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *inst_per_s);
 // dynamic shared memory per block of the kernel the plan selects (0 for the generic kernels' own sizing): crf_plan_info
 size_t rates_dynamic_smem(const DevTables &m);

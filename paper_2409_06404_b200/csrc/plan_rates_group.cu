@@ -312,7 +312,8 @@ RatesGroupPlanOffsets build_rates_group_plan(const crf_tables *t, const crf_plan
         chunks = make_chunks(B, n_chunks, W);
         Rc = 0;
         for (const Chunk &c : chunks) Rc = std::max(Rc, (int)c.rx.size());
-        q_rows = std::max(Rc + 1, tm ? W + Ns + 1 : W);
+        q_rows = std::max(Rc + 1, tm ? W + Ns + 1 : 3 * W);  // (the epilogue reduces three block-wide sums: 3 W rows)
+        q_rows = std::max(q_rows, 3 * W);
         blocks.clear();
         stage_bytes = 0;
         for (const Chunk &c : chunks) {
@@ -346,7 +347,7 @@ RatesGroupPlanOffsets build_rates_group_plan(const crf_tables *t, const crf_plan
             g[4] = -s * A(4) / 20.0, g[5] = s * A(5), g[6] = -s * A(6);
             h[0] = A(0), h[1] = A(1) / 2.0, h[2] = A(2) / 3.0, h[3] = A(3) / 4.0, h[4] = A(4) / 5.0, h[5] = A(5);
             if (rg == 0) g[7] = t->Tmid[k], h[7] = t->Tmid[k];
-            if (rg == 1) g[7] = 1.0 / t->W[k];
+            if (rg == 1) g[7] = 1.0 / t->W[k], h[7] = 1.0 / t->W[k];
         }
     o.chunk = b.add(cdesc), o.stage = b.add(stage), o.gco = b.add(gco), o.hco = b.add(hco), o.own = b.add(own);
     return o;

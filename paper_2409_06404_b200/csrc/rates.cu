@@ -159,7 +159,7 @@ cudaError_t launch_rates(const DevTables &m, const double *T, const double *p, c
                          double *omega, double *qdot, cudaStream_t st)
 {
     if (m.rs.W > 0) return launch_rates_smem(m, T, p, Y, n, omega, qdot, st);
-    if (m.rg.W > 0) return launch_rates_group(m, T, p, Y, n, omega, qdot, st);
+    if (m.rg.W > 0) return launch_rates_group(m, rates_io(T, p, Y, omega, qdot), n, st);
     if (m.rp.W > 0) return launch_rates_staged(m, T, p, Y, n, omega, qdot, st);
     const size_t per_thread = sizeof(double) * 2 * (size_t)m.Ns;
     const size_t budget = 100 * 1024;  // two blocks per SM

@@ -130,6 +130,37 @@ __device__ __forceinline__ void store_row(double *__restrict__ row, int64_t i0, 
     }
 }
 
+// input row of the lane: mode 0 the PPL adjacent points of `a`; mode 1 (a[i], b[i]); mode 2 (a[i], a[i] + sigma b[i])
+// (b null = no perturbation), one rounding per operation so that the perturbed state is the one a host forms
+template <int PPL>
+__device__ __forceinline__ void in_row(const RatesIO &io, const double *__restrict__ a, const double *__restrict__ b,
+                                       int64_t i0, int64_t n, bool vec, double (&v)[PPL])
+{
+    if (io.mode == 0) {
+        load_row<PPL>(a, i0, n, vec, v);
+        return;
+    }
+    const int64_t i = min(i0, n - 1);
+    v[0] = a[i];
+    if (io.mode == 1)
+        v[PPL - 1] = b[i];
+    else
+        v[PPL - 1] = b ? __dadd_rn(v[0], __dmul_rn(io.sigma, b[i])) : v[0];
+}
+// output rows: mode 0 -> a; mode 1: v[0] -> a, v[1] -> b; mode 2: v[0] -> a (if given), (v[1] - v[0]) / sigma -> b
+template <int PPL>
+__device__ __forceinline__ void out_rows(const RatesIO &io, double *__restrict__ a, double *__restrict__ b, int64_t off,
+                                         int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
+{
+    if (io.mode == 0) {
+        store_row<PPL>(a + off, i0, n, vec, v);
+        return;
+    }
+    if (i0 >= n) return;
+    if (a) a[off + i0] = v[0];
+    b[off + i0] = io.mode == 1 ? v[PPL - 1] : __ddiv_rn(__dsub_rn(v[PPL - 1], v[0]), io.sigma);
+}
+
 // ---- bulk copy global -> shared with mbarrier completion (TMA, non-tensor form) ------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
@@ -380,8 +411,7 @@ __device__ __forceinline__ double nasa_eval(const double2 *set, double Tu, doubl
 
 template <int W, int PPL, int MAXOWN, bool TM>
 __global__ void __launch_bounds__(32 * W, 16 / W)
-    rates_group_kernel(DevTables m, const double *__restrict__ T, const double *__restrict__ p,
-                       const double *__restrict__ Y, int64_t n, double *__restrict__ omega, double *__restrict__ qdot)
+    rates_group_kernel(DevTables m, RatesIO io, int64_t n)
 {
     extern __shared__ double2 sm2[];
     __shared__ uint64_t mbar[2];
@@ -421,18 +451,21 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     }
     const unsigned tmq = TM ? sTmBase + (((unsigned)(warp & 3) * 32u) << 16) : 0u;
 
-    const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * PPL;
+    // mode 0: the lane's PPL points are adjacent grid points; modes 1, 2 (PPL = 2): the lane's two "points" are the two
+    // states of ONE grid point, so tables, records and lists are read once for both evaluations
+    const int mode = io.mode;
+    const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * (mode == 0 ? PPL : 1);
     const bool vec = (n & 1) == 0;
     Ctx<PPL> c;
     double pi[PPL];
-    load_row<PPL>(T, i0, n, vec, c.T);
-    load_row<PPL>(p, i0, n, vec, pi);
+    in_row<PPL>(io, io.T, io.T2, i0, n, vec, c.T);
+    in_row<PPL>(io, io.p, io.p2, i0, n, vec, pi);
     // ---- a1: Z_k = Y_k / W_k; warp w takes species w, w + W, ...: all row loads of the warp are in flight together
     double z[MAXOWN][PPL];
 #pragma unroll
     for (int s = 0; s < MAXOWN; ++s) {
         const int k = warp + W * s;
-        if (k < Ns) load_row<PPL>(Y + (int64_t)k * n, i0, n, vec, z[s]);
+        if (k < Ns) in_row<PPL>(io, io.Y + (int64_t)k * n, io.Y2 ? io.Y2 + (int64_t)k * n : nullptr, i0, n, vec, z[s]);
     }
     double lc02[PPL], omL[PPL];
 #pragma unroll
@@ -472,6 +505,14 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
 #pragma unroll
         for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
         rho[u] = pi[u] / (CRF_R_GAS * c.T[u] * s);
+        invW[u] = s;
+    }
+    if (warp == 0 && mode == 0 && (io.rho || io.Wbar)) {  // by-products of crf_rhs_pointwise (Eq. 1d)
+        double wb[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) wb[u] = 1.0 / invW[u];
+        if (io.rho) store_row<PPL>(io.rho, i0, n, vec, rho);
+        if (io.Wbar) store_row<PPL>(io.Wbar, i0, n, vec, wb);
     }
     // ---- a2: d_k = 2^(log2(p_ref/RT) - log2e g_k/RT), u_k = rho Z_k / d_k
     char *uDst = (TM ? sUtmp : sS + (size_t)(Ns + 1) * RB) + lane * LB;
@@ -563,23 +604,55 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     // ---- store omega; a9: qdot = -sum_k h_k omega_k
     mbar_wait(&mbar[nch & 1], (unsigned)((nch >> 1) + (nch & 1)) & 1u);
     const double2 *sH = reinterpret_cast<const double2 *>(sStage + (size_t)(nch & 1) * sb);
-    double qd[PPL];
+    const bool emit = mode == 0 && (io.cp || io.h || io.cpk);
+    double qd[PPL], cpm[PPL], hm[PPL];
 #pragma unroll
-    for (int u = 0; u < PPL; ++u) qd[u] = 0.0;
+    for (int u = 0; u < PPL; ++u) qd[u] = cpm[u] = hm[u] = 0.0;
 #pragma unroll
     for (int s = 0; s < MAXOWN; ++s) {
         const int k = __ldg(rg.own + warp * MAXOWN + s);
         if (k >= 0) {
             const double2 *h = sH + 8 * k;
             const double Tmid = h[3].y;
+            double hk[PPL];
 #pragma unroll
-            for (int u = 0; u < PPL; ++u)
-                qd[u] = fma(-nasa_eval<false>(h, c.T[u], c.rT[u], 0.0, Tmid), om[s][u], qd[u]);
-            store_row<PPL>(omega + (int64_t)k * n, i0, n, vec, om[s]);
+            for (int u = 0; u < PPL; ++u) {
+                hk[u] = nasa_eval<false>(h, c.T[u], c.rT[u], 0.0, Tmid);
+                qd[u] = fma(-hk[u], om[s][u], qd[u]);
+            }
+            out_rows<PPL>(io, io.omega, io.omega2, (int64_t)k * n, i0, n, vec, om[s]);
+            if (emit) {
+                // crf_rhs_pointwise: c_pk/R from the h/(RT) set (a_i = (i + 1) c_i), mixture c_p and h; the Y row is
+                // read again (it was consumed by the species this warp handled in the prologue, not the ones it owns)
+                double y[PPL], cpk[PPL];
+                load_row<PPL>(io.Y + (int64_t)k * n, i0, n, vec, y);
+                const double rW = h[7].y;
+#pragma unroll
+                for (int u = 0; u < PPL; ++u) {
+                    const double2 *g = h + (c.T[u] <= Tmid ? 0 : 4);
+                    const double2 c01 = g[0], c23 = g[1], c45 = g[2];
+                    double v = fma(c.T[u], 5.0 * c45.x, 4.0 * c23.y);
+                    v = fma(c.T[u], v, 3.0 * c23.x);
+                    v = fma(c.T[u], v, 2.0 * c01.y);
+                    v = fma(c.T[u], v, c01.x);
+                    const double zk = y[u] * rW;
+                    cpm[u] = fma(zk, v, cpm[u]);
+                    hm[u] = fma(zk, hk[u], hm[u]);
+                    cpk[u] = v * CRF_R_GAS;
+                }
+                if (io.cpk) store_row<PPL>(io.cpk + (int64_t)k * n, i0, n, vec, cpk);
+            }
         }
     }
+    // block-wide sums of qdot (and c_p, h): [3][W][PPL][32] in the q buffer
 #pragma unroll
-    for (int u = 0; u < PPL; ++u) sred[(warp * PPL + u) * 32 + lane] = qd[u];
+    for (int u = 0; u < PPL; ++u) {
+        sred[(warp * PPL + u) * 32 + lane] = qd[u];
+        if (emit) {
+            sred[((W + warp) * PPL + u) * 32 + lane] = cpm[u];
+            sred[((2 * W + warp) * PPL + u) * 32 + lane] = hm[u];
+        }
+    }
     __syncthreads();
     if (warp == 0) {
         double out[PPL];
@@ -590,39 +663,52 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
             for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
             out[u] = s * (CRF_R_GAS * c.T[u]);
         }
-        store_row<PPL>(qdot, i0, n, vec, out);
+        out_rows<PPL>(io, io.qdot, io.qdot2, 0, i0, n, vec, out);
         if (TM)
             asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(sTmBase), "r"((unsigned)rg.tm_cols)
                          : "memory");
     }
+    if (warp == 1 && emit) {
+        double oc[PPL], oh[PPL];
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) {
+            double sc = 0.0, sh = 0.0;
+#pragma unroll
+            for (int w = 0; w < W; ++w) {
+                sc += sred[((W + w) * PPL + u) * 32 + lane];
+                sh += sred[((2 * W + w) * PPL + u) * 32 + lane];
+            }
+            oc[u] = sc * CRF_R_GAS;
+            oh[u] = sh * (CRF_R_GAS * c.T[u]);
+        }
+        if (io.cp) store_row<PPL>(io.cp, i0, n, vec, oc);
+        if (io.h) store_row<PPL>(io.h, i0, n, vec, oh);
+    }
 }
 
 template <int W, int PPL, int MAXOWN, bool TM>
-cudaError_t launch_k(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
-                     double *qdot, cudaStream_t st)
+cudaError_t launch_k(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
 {
     const size_t smem = rates_group_dynamic_smem(m);
     cudaError_t e = cudaFuncSetAttribute(rates_group_kernel<W, PPL, MAXOWN, TM>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const int64_t per_block = 32 * PPL;
-    rates_group_kernel<W, PPL, MAXOWN, TM>
-        <<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, p, Y, n, omega, qdot);
+    const int64_t per_block = io.mode == 0 ? 32 * PPL : 32;
+    rates_group_kernel<W, PPL, MAXOWN, TM><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, io, n);
     crf_count_launch();
     return cudaGetLastError();
 }
 
 template <int W, int PPL>
-cudaError_t launch_wp(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
-                      double *qdot, cudaStream_t st)
+cudaError_t launch_wp(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
 {
     switch (m.rg.maxown * 2 + (m.rg.tm_cols > 0)) {
-    case 8: return launch_k<W, PPL, 4, false>(m, T, p, Y, n, omega, qdot, st);
-    case 9: return launch_k<W, PPL, 4, true>(m, T, p, Y, n, omega, qdot, st);
-    case 16: return launch_k<W, PPL, 8, false>(m, T, p, Y, n, omega, qdot, st);
-    case 17: return launch_k<W, PPL, 8, true>(m, T, p, Y, n, omega, qdot, st);
-    case 32: return launch_k<W, PPL, 16, false>(m, T, p, Y, n, omega, qdot, st);
-    case 33: return launch_k<W, PPL, 16, true>(m, T, p, Y, n, omega, qdot, st);
+    case 8: return launch_k<W, PPL, 4, false>(m, io, n, st);
+    case 9: return launch_k<W, PPL, 4, true>(m, io, n, st);
+    case 16: return launch_k<W, PPL, 8, false>(m, io, n, st);
+    case 17: return launch_k<W, PPL, 8, true>(m, io, n, st);
+    case 32: return launch_k<W, PPL, 16, false>(m, io, n, st);
+    case 33: return launch_k<W, PPL, 16, true>(m, io, n, st);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -636,16 +722,17 @@ size_t rates_group_dynamic_smem(const DevTables &m)
     return (size_t)(m.Ns + 1) * (rg.tm_cols > 0 ? 1 : 2) * rb + (size_t)rg.q_rows * rb + 2 * (size_t)rg.stage_bytes;
 }
 
-cudaError_t launch_rates_group(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
-                               double *omega, double *qdot, cudaStream_t st)
+// io.mode 1 and 2 need a plan with two points per lane (the two states of a grid point share a lane)
+cudaError_t launch_rates_group(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
 {
+    if (io.mode != 0 && m.rg.PPL != 2) return cudaErrorInvalidValue;
     switch (m.rg.W * 10 + m.rg.PPL) {
-    case 41: return launch_wp<4, 1>(m, T, p, Y, n, omega, qdot, st);
-    case 42: return launch_wp<4, 2>(m, T, p, Y, n, omega, qdot, st);
-    case 81: return launch_wp<8, 1>(m, T, p, Y, n, omega, qdot, st);
-    case 82: return launch_wp<8, 2>(m, T, p, Y, n, omega, qdot, st);
-    case 161: return launch_wp<16, 1>(m, T, p, Y, n, omega, qdot, st);
-    case 162: return launch_wp<16, 2>(m, T, p, Y, n, omega, qdot, st);
+    case 41: return launch_wp<4, 1>(m, io, n, st);
+    case 42: return launch_wp<4, 2>(m, io, n, st);
+    case 81: return launch_wp<8, 1>(m, io, n, st);
+    case 82: return launch_wp<8, 2>(m, io, n, st);
+    case 161: return launch_wp<16, 1>(m, io, n, st);
+    case 162: return launch_wp<16, 2>(m, io, n, st);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -150,7 +150,28 @@ __global__ void __launch_bounds__(TB) thermo_species_kernel(DevTables m, const d
     }
 }
 
+// rho = p Wbar / (R T), Wbar = 1 / sum_k Y_k / W_k (the unfused path of crf_rhs_pointwise)
+__global__ void __launch_bounds__(TB) density_kernel(DevTables m, const double *__restrict__ T, const double *__restrict__ p,
+                                                     const double *__restrict__ Y, int64_t n, double *__restrict__ rho,
+                                                     double *__restrict__ Wbar)
+{
+    const int64_t i = (int64_t)blockIdx.x * TB + threadIdx.x;
+    if (i >= n) return;
+    double iw = 0.0;
+    for (int k = 0; k < m.Ns; ++k) iw = fma(Y[(int64_t)k * n + i], __ldg(m.rW + k), iw);
+    if (Wbar) Wbar[i] = 1.0 / iw;
+    if (rho) rho[i] = p[i] / (CRF_R_GAS * T[i] * iw);
+}
+
 }  // namespace
+
+cudaError_t launch_density(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *rho,
+                           double *Wbar, cudaStream_t st)
+{
+    density_kernel<<<(unsigned)((n + TB - 1) / TB), TB, 0, st>>>(m, T, p, Y, n, rho, Wbar);
+    crf_count_launch();
+    return cudaGetLastError();
+}
 
 cudaError_t launch_thermo(const DevTables &m, const double *T, const double *Y, int64_t n, double *cp, double *h,
                           cudaStream_t st)

@@ -1,0 +1,152 @@
+"""GPU parity of the SURVEY.md 8(f) rows built on the hot path: crf_rhs_pointwise (row 1: the fused right-hand-side
+evaluation with its by-products rho, Wbar, c_pk), crf_production_rates_pair and crf_production_rates_jv (row 2: two
+states per launch and the difference quotient of the Jacobian-vector product).  All through the C ABI, against the
+oracle on the same seeded inputs, at BASELINE.json's tolerances (the quotient: the tolerance of two evaluations
+divided by sigma)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2409_06404_b200 import workloads as wl
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+SMALL_N = {"C1": 512, "C2": 2 * 1024 + 333, "C3": 3 * 1024 + 77, "C4": 1024 + 301, "C5": 512 + 129}
+
+
+@pytest.fixture(scope="module")
+def binding():
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2409_06404_b200 import binding as b
+    b.lib()
+    return b
+
+
+def _np(d):
+    return {k: (v.cpu().numpy() if v is not None else None) for k, v in d.items()}
+
+
+def _check_rhs(out, ref, what):
+    e = parity.assert_parity(out, ref, what)
+    for key in ("cpk", "rho", "Wbar"):
+        err = float(np.max(np.abs(out[key] - ref[key]) / np.abs(ref[key])))
+        assert err <= parity.RTOL, f"{what}: {key} relative error {err:.3g}"
+        e[key] = err / parity.RTOL
+    return e
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+@pytest.mark.parametrize("odd", [0, 1])
+def test_rhs_pointwise(binding, oracle_mod, name, odd):
+    desc = wl.make_mechanism(name)
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    n = SMALL_N[name] + odd
+    st = wl.make_state(name, n=n, total=n)
+    d = parity.to_dev(st)
+    out = _np(gm.rhs_pointwise(d["T"], d["p"], d["Y"]))
+    e = _check_rhs(out, om.rhs_pointwise(**st), f"rhs {name} n={n}")
+    print(name, n, {k: f"{v:.3g}" for k, v in e.items()})
+    # the outputs shared with the three separate calls are the same numbers within the same tolerances, and the
+    # by-products may be skipped
+    out2 = _np(gm.rhs_pointwise(d["T"], d["p"], d["Y"], want_cpk=False))
+    assert out2["cpk"] is None and np.array_equal(out2["omega"], out["omega"]) and np.array_equal(out2["cp"], out["cp"])
+
+
+@pytest.mark.parametrize("opt", [dict(rates_kernel="staged"), dict(rates_kernel="generic"), dict(rates_kernel="group", rates_tmem=1),
+                                 dict(rates_kernel="group", rates_PPL=1)],
+                         ids=lambda o: ",".join(f"{k}={v}" for k, v in o.items()))
+def test_rhs_pointwise_other_plans(binding, oracle_mod, opt):
+    """Mechanisms without a warp-group plan take the separate kernels; u rows in shared memory and one point per lane
+    emit the same by-products."""
+    desc = wl.make_mechanism("C3")
+    gm, om = binding.Mechanism(desc, options=opt), oracle_mod.Oracle(desc)
+    n = 1025
+    st = wl.make_state("C3", n=n, total=n)
+    d = parity.to_dev(st)
+    _check_rhs(_np(gm.rhs_pointwise(d["T"], d["p"], d["Y"])), om.rhs_pointwise(**st), f"rhs C3 {opt}")
+
+
+def _two_states(name, n):
+    a = wl.make_state(name, n=n, total=2 * n)
+    b = wl.make_state(name, n=n, offset=n, total=2 * n)
+    return a, b
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_pair_matches_oracle_and_single_calls(binding, oracle_mod, name):
+    desc = wl.make_mechanism(name)
+    gm = binding.Mechanism(desc, options=dict(rates_kernel="group"))
+    om = oracle_mod.Oracle(desc)
+    n = SMALL_N[name]
+    a, b = _two_states(name, n)
+    da, db = parity.to_dev(a), parity.to_dev(b)
+    o1, q1, o2, q2 = gm.production_rates_pair(da["T"], da["p"], da["Y"], db["T"], db["p"], db["Y"])
+    ref = om.production_rates_pair(a["T"], a["p"], a["Y"], b["T"], b["p"], b["Y"])
+    for got, key, sk in ((o1, "omega", "S_omega"), (q1, "qdot", "S_q"), (o2, "omega2", "S_omega2"), (q2, "qdot2", "S_q2")):
+        err = np.max(np.abs(got.cpu().numpy() - ref[key]) / (parity.RATE_TOL * ref[sk] + 1e-30))
+        assert err <= 1.0, (name, key, err)
+    # one launch for two states = two launches of the same kernel, bit for bit
+    s1, sq1 = gm.production_rates(da["T"], da["p"], da["Y"])
+    s2, sq2 = gm.production_rates(db["T"], db["p"], db["Y"])
+    assert torch.equal(o1, s1) and torch.equal(q1, sq1) and torch.equal(o2, s2) and torch.equal(q2, sq2)
+
+
+def test_pair_without_a_shared_launch(binding, oracle_mod):
+    """A plan that cannot hold two states per lane answers the pair call with two launches: same numbers."""
+    desc = wl.make_mechanism("C3")
+    gm, om = binding.Mechanism(desc, options=dict(rates_kernel="staged")), oracle_mod.Oracle(desc)
+    a, b = _two_states("C3", 777)
+    da, db = parity.to_dev(a), parity.to_dev(b)
+    o1, q1, o2, q2 = gm.production_rates_pair(da["T"], da["p"], da["Y"], db["T"], db["p"], db["Y"])
+    ref = om.production_rates_pair(a["T"], a["p"], a["Y"], b["T"], b["p"], b["Y"])
+    assert np.max(np.abs(o2.cpu().numpy() - ref["omega2"]) / (parity.RATE_TOL * ref["S_omega2"] + 1e-30)) <= 1.0
+    assert np.max(np.abs(o1.cpu().numpy() - ref["omega"]) / (parity.RATE_TOL * ref["S_omega"] + 1e-30)) <= 1.0
+    with pytest.raises(binding.CrfError, match="no warp-group plan"):
+        gm.production_rates_jv(da["T"], da["p"], da["Y"], db["T"], db["p"], db["Y"], 1e-6)
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+@pytest.mark.parametrize("sigma", [1e-3, -1e-7])
+def test_jv_difference_quotient(binding, oracle_mod, name, sigma):
+    """(omega(y + sigma v) - omega(y)) / sigma, perturbation formed in the kernel: the direction is a seeded random
+    vector scaled like the state (the perturbation factor of [17], would scale it the same way)."""
+    desc = wl.make_mechanism(name)
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)  # default plan: the call uses the warp-group plan
+    n = SMALL_N[name] + 1
+    st = wl.make_state(name, n=n, total=n)
+    rng = np.random.default_rng(42)
+    v = dict(dT=st["T"] * rng.uniform(-1, 1, n), dp=st["p"] * rng.uniform(-1, 1, n),
+             dY=st["Y"] * rng.uniform(-1, 1, st["Y"].shape))
+    d, dv = parity.to_dev(st), parity.to_dev(v)
+    om_b, qd_b, Jo, Jq = gm.production_rates_jv(d["T"], d["p"], d["Y"], dv["dT"], dv["dp"], dv["dY"], sigma)
+    ref = om.production_rates_jv(st["T"], st["p"], st["Y"], v["dT"], v["dp"], v["dY"], sigma)
+    e = {}
+    for got, key, sk in ((om_b, "omega", "S_omega"), (qd_b, "qdot", "S_q"), (Jo, "Jomega", "S_Jomega"), (Jq, "Jqdot", "S_Jqdot")):
+        e[key] = float(np.max(np.abs(got.cpu().numpy() - ref[key]) / (parity.RATE_TOL * ref[sk] + 1e-30 / abs(sigma))))
+        assert e[key] <= 1.0, (name, key, e)
+    print(name, sigma, {k: f"{x:.3g}" for k, x in e.items()})
+    # the quotient alone (no base outputs), and without a pressure perturbation
+    _, _, Jo2, Jq2 = gm.production_rates_jv(d["T"], d["p"], d["Y"], dv["dT"], dv["dp"], dv["dY"], sigma, base=False)
+    assert torch.equal(Jo2, Jo) and torch.equal(Jq2, Jq)
+    _, _, Jo3, _ = gm.production_rates_jv(d["T"], d["p"], d["Y"], dv["dT"], None, dv["dY"], sigma)
+    ref3 = om.production_rates_jv(st["T"], st["p"], st["Y"], v["dT"], np.zeros(n), v["dY"], sigma)
+    assert np.max(np.abs(Jo3.cpu().numpy() - ref3["Jomega"]) / (parity.RATE_TOL * ref3["S_Jomega"] + 1e-30 / abs(sigma))) <= 1.0
+
+
+def test_new_calls_reject_bad_arguments(binding):
+    desc = wl.make_mechanism("C1")
+    gm = binding.Mechanism(desc)
+    st = parity.to_dev(wl.make_state("C1", n=64, total=64))
+    with pytest.raises(binding.CrfError, match="sigma"):
+        gm.production_rates_jv(st["T"], st["p"], st["Y"], st["T"], st["p"], st["Y"], 0.0)
+    L = binding.lib()
+    z = torch.zeros(64 * 9 + 8, dtype=torch.float64, device="cuda")
+    args = [gm._h, st["T"].data_ptr(), st["p"].data_ptr(), st["Y"].data_ptr(), 64]
+    outs = [z.data_ptr()] * 10
+    assert L.crf_rhs_pointwise(*args, *outs) == 0
+    outs[0] = z.data_ptr() + 8
+    assert L.crf_rhs_pointwise(*args, *outs) == -1  # misaligned
+    outs[0] = None
+    assert L.crf_rhs_pointwise(*args, *outs) == -1  # omega is required
+    assert L.crf_rhs_pointwise(gm._h, st["T"].data_ptr(), st["p"].data_ptr(), st["Y"].data_ptr(), 0, *([None] * 10)) == 0
