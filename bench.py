@@ -41,6 +41,9 @@ def parse():
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--points", type=int, default=0, help="override the number of points (debug)")
     ap.add_argument("--cpu-points", type=int, default=0, help="oracle sample size (default: ~10-30 s of CPU)")
+    ap.add_argument("--path", default="three", choices=["three", "rhs", "jv"],
+                    help="three: crf_thermo + crf_production_rates + crf_mix_transport (the default step); rhs: one "
+                         "crf_rhs_pointwise call (SURVEY 8(f)1); jv: one crf_production_rates_jv call (8(f)2)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -50,13 +53,17 @@ def parse():
 CPU_SAMPLE = {"C1": 512, "C2": 1 << 20, "C3": 1 << 19, "C4": 1 << 18, "C5": 1 << 16}
 
 
-def config_dict(name, n, world):
+CALLS = {"three": ["crf_thermo", "crf_production_rates", "crf_mix_transport"], "rhs": ["crf_rhs_pointwise"],
+         "jv": ["crf_production_rates_jv"]}
+
+
+def config_dict(name, n, world, path="three"):
     from paper_2409_06404_b200 import workloads as wl
     c = wl.CONFIGS[name]
     return {"workload": f"{name} (BASELINE.json configs[{int(name[1]) - 1}])", "Ns": c["Ns"], "Nr": c["Nr"],
             "N3": c["N3"], "Nt": c["Nt"], "points_per_gpu": n, "elements_per_gpu": n // 512,
             "state": c["state"], "seed": c["seed"], "parallelism": f"points x{world} (no collective)",
-            "calls_per_step": ["crf_thermo", "crf_production_rates", "crf_mix_transport"],
+            "calls_per_step": CALLS[path],
             "l2": "inputs exceed L2 (no flush needed)" if n * 8 * (c["Ns"] + 2) > 126e6 * 2 else "flushed between steps"}
 
 
@@ -191,6 +198,108 @@ def host_cores_for_the_oracle():
         os.environ.pop("OMP_NUM_THREADS")
 
 
+def other_path(args, mech, dev, out, n, name, world, rank, local, barrier, flush, stream):
+    """--path rhs | jv: the SURVEY 8(f) calls on the same workload, with the separate-call equivalent timed beside
+    them in the same run (CUDA events on the launching stream, K steps each, max over ranks)."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_2409_06404_b200 import binding, rooflines
+    from paper_2409_06404_b200 import workloads as wl
+    Ns = mech.Ns
+    f64 = dict(dtype=torch.float64, device="cuda")
+    cfg = wl.CONFIGS[name]
+    n_eff = int(mech.tables.arrays["eff_ptr"][-1])
+    w_th, w_ra, w_tr = (rooflines.thermo_work(Ns), rooflines.rates_work(Ns, cfg["Nr"], cfg["N3"], cfg["Nt"], n_eff),
+                        rooflines.transport_work(Ns))
+    if args.path == "rhs":
+        out.update(cpk=torch.empty(Ns, n, **f64), rho=torch.empty(n, **f64), Wbar=torch.empty(n, **f64))
+
+        def fused():
+            mech.rhs_pointwise(dev["T"], dev["p"], dev["Y"], out)
+
+        def separate():  # what a caller does without the fused call: the three calls (no rho, Wbar, c_pk at all)
+            mech.thermo(dev["T"], dev["p"], dev["Y"], out["cp"], out["h"])
+            mech.production_rates(dev["T"], dev["p"], dev["Y"], out["omega"], out["qdot"])
+            mech.mix_transport(dev["T"], dev["p"], dev["Y"], out["mu"], out["lam"], out["rhoD"])
+        flops = w_th["F"] + w_ra["F"] + w_tr["F"]
+        alg_bytes = 8 * (Ns + 2) + 8 * (3 * Ns + 7)  # one read of T, p, Y; omega, rhoD, c_pk rows and 7 scalar fields
+        sep_name, sep_note = "three_calls", "crf_thermo + crf_production_rates + crf_mix_transport (no rho, Wbar, c_pk)"
+    else:
+        gen = torch.Generator(device="cuda").manual_seed(1234 + rank)
+        v = {k: dev[k] * (2 * torch.rand(dev[k].shape, generator=gen, **f64) - 1) for k in ("T", "p", "Y")}
+        sigma = 1e-6
+        Jo, Jq = torch.empty(Ns, n, **f64), torch.empty(n, **f64)
+        pert = {k: torch.empty_like(dev[k]) for k in ("T", "p", "Y")}
+        om2, qd2 = torch.empty(Ns, n, **f64), torch.empty(n, **f64)
+
+        def fused():
+            mech.production_rates_jv(dev["T"], dev["p"], dev["Y"], v["T"], v["p"], v["Y"], sigma,
+                                     out=(out["omega"], out["qdot"], Jo, Jq))
+
+        def separate():  # perturb (3 axpy), two crf_production_rates calls, two quotients
+            for k in ("T", "p", "Y"):
+                torch.add(dev[k], v[k], alpha=sigma, out=pert[k])
+            mech.production_rates(dev["T"], dev["p"], dev["Y"], out["omega"], out["qdot"])
+            mech.production_rates(pert["T"], pert["p"], pert["Y"], om2, qd2)
+            torch.sub(om2, out["omega"], out=Jo).div_(sigma)
+            torch.sub(qd2, out["qdot"], out=Jq).div_(sigma)
+        flops = 2 * w_ra["F"]
+        alg_bytes = 8 * 2 * (Ns + 2) + 8 * 2 * (Ns + 1)
+        sep_name, sep_note = "separate_calls", "3 axpy + 2 crf_production_rates + 2 quotient kernels (torch elementwise)"
+
+    K = max(args.steps, 1)
+
+    def timed(fn):
+        for _ in range(max(args.warmup, 3)):
+            fn()
+        barrier()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+        ev[0].record(stream)
+        for k in range(K):
+            if flush is not None:
+                flush.add_(1)
+            fn()
+            ev[k + 1].record(stream)
+        barrier()
+        ms = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(K)])
+        t = torch.tensor([float(ms.mean())], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item()), float(np.median(ms)), float(ms.min())
+
+    clocks = ClockSampler(local) if rank == 0 else None
+    launches0 = binding.launch_count()
+    ms, med, best = timed(fused)
+    launches = (binding.launch_count() - launches0) * K // (K + max(args.warmup, 3))
+    clock_info = clocks.stop() if clocks else None
+    sep_ms, sep_med, sep_best = timed(separate)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+    peaks = rooflines.measured_peaks(ROOT)
+    t_alu = flops * n / (rooflines.FP64_PEAK_TFLOPS * 1e12)
+    t_hbm = alg_bytes * n / (peaks["hbm_gbs"] * 1e9)
+    call = CALLS[args.path][0]
+    roof = {"bound": "alu" if t_alu >= t_hbm else "hbm", "kernel": call, "achieved": flops * n / (ms * 1e-3) / 1e12,
+            "peak": rooflines.FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": max(t_alu, t_hbm) / (ms * 1e-3), "traffic": None,
+            "peak_source": "148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md); FMA = 2 flops",
+            "flops_per_point": flops, "bytes_per_point": alg_bytes, "t_hbm_ms": 1e3 * t_hbm, "t_alu_ms": 1e3 * t_alu}
+    line = {"metric": METRIC, "value": world * n / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms, "ms_median": med, "ms_best": best, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(name, n, world, args.path), "clocks": clock_info, "e2e": None,
+            "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": None,
+            sep_name: {"ms_per_step": sep_ms, "ms_median": sep_med, "ms_best": sep_best, "what": sep_note,
+                       "fused_over_separate": ms / sep_ms}}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     args = parse()
     host_cores_for_the_oracle()
@@ -251,6 +360,9 @@ def main():
         mech.mix_transport(dev["T"], dev["p"], dev["Y"], out["mu"], out["lam"], out["rhoD"])
         if ev:
             ev[3].record(stream)
+
+    if args.path != "three":
+        return other_path(args, mech, dev, out, n, name, world, rank, local, barrier, flush, stream)
 
     for _ in range(max(args.warmup, 3)):
         step()

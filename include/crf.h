@@ -168,7 +168,7 @@ int crf_production_rates_pair(const crf_mech *mech, const double *T, const doubl
 
 /* The difference quotient itself: the perturbed state y' = (T + sigma dT, p + sigma dp, Y + sigma dY) is formed in
  * the kernel (multiply, then add: one rounding each, as a host would), both states are evaluated in one launch and
- *   Jomega[Ns*n] = (omega(y') - omega(y)) / sigma,   Jqdot[n] = (qdot(y') - qdot(y)) / sigma
+ *   Jomega[Ns*n] = (omega(y') - omega(y)) (1/sigma),   Jqdot[n] = (qdot(y') - qdot(y)) (1/sigma)
  * are returned next to omega(y), qdot(y) (omega and qdot may both be NULL).  dp may be NULL (no pressure
  * perturbation).  sigma must be finite and non-zero.  Each value of the quotient carries the rounding of two
  * evaluations divided by sigma: its tolerance scale is (S(y) + S(y')) / |sigma|.  CRF_EUNSUPPORTED for a mechanism

@@ -394,7 +394,8 @@ int crf_production_rates_jv(const crf_mech *mech, const double *T, const double 
         return fail(CRF_EUNSUPPORTED, "crf_production_rates_jv: this mechanism has no warp-group plan with two states per lane "
                                       "(use crf_production_rates_pair on a perturbed copy)");
     RatesIO io = rates_io(T, p, Y, omega, qdot);
-    io.T2 = dT, io.p2 = dp, io.Y2 = dY, io.omega2 = Jomega, io.qdot2 = Jqdot, io.sigma = sigma, io.mode = 2;
+    io.T2 = dT, io.Y2 = dY, io.omega2 = Jomega, io.qdot2 = Jqdot, io.sigma = sigma, io.inv_sigma = 1.0 / sigma, io.mode = 2;
+    io.p2 = dp ? dp : p, io.sigma_p = dp ? sigma : 0.0;  // (no pressure perturbation: p + 0 p)
     cudaError_t e = launch_rates_group(mech->dev, io, n, mech->stream);
     return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_production_rates_jv");
 }

@@ -7,12 +7,12 @@ void crf_count_launch();
 // What one launch of the production-rates kernels reads and writes (device pointers).
 //   mode 0  omega, qdot at (T, p, Y); optionally the thermodynamic by-products of the same pass (crf_rhs_pointwise)
 //   mode 1  two states of the same points in one launch: (T, p, Y) -> omega, qdot and (T2, p2, Y2) -> omega2, qdot2
-//   mode 2  difference quotient: second state = (T, p, Y) + sigma (T2, p2, Y2) formed in the kernel (p2 may be null = 0);
-//           omega, qdot of the base state (may be null) and omega2, qdot2 = (f(second) - f(base)) / sigma
+//   mode 2  difference quotient: second state = (T, p, Y) + (sigma T2, sigma_p p2, sigma Y2) formed in the kernel;
+//           omega, qdot of the base state (may be null) and omega2, qdot2 = (f(second) - f(base)) (1/sigma)
 struct RatesIO {
     const double *T, *p, *Y;
     const double *T2, *p2, *Y2;
-    double sigma;
+    double sigma, sigma_p, inv_sigma;  // (sigma_p: the step applied to p2; 0 when the caller gave no dp)
     int mode;
     double *omega, *qdot;
     double *omega2, *qdot2;
@@ -22,6 +22,7 @@ inline RatesIO rates_io(const double *T, const double *p, const double *Y, doubl
 {
     RatesIO io{};
     io.T = T, io.p = p, io.Y = Y, io.omega = omega, io.qdot = qdot;
+    io.T2 = T, io.p2 = p, io.Y2 = Y;  // (never null: the kernels form row pointers from them in every mode)
     return io;
 }
 

@@ -130,35 +130,33 @@ __device__ __forceinline__ void store_row(double *__restrict__ row, int64_t i0, 
     }
 }
 
-// input row of the lane: mode 0 the PPL adjacent points of `a`; mode 1 (a[i], b[i]); mode 2 (a[i], a[i] + sigma b[i])
-// (b null = no perturbation), one rounding per operation so that the perturbed state is the one a host forms
-template <int PPL>
+// input row of the lane: MODE 0 the PPL adjacent points of `a`; MODE 1 (a[i], b[i]); MODE 2 (a[i], a[i] + sigma b[i]),
+// one rounding per operation so that the perturbed state is the one a host forms
+template <int PPL, int MODE>
 __device__ __forceinline__ void in_row(const RatesIO &io, const double *__restrict__ a, const double *__restrict__ b,
-                                       int64_t i0, int64_t n, bool vec, double (&v)[PPL])
+                                       double sigma, int64_t i0, int64_t n, bool vec, double (&v)[PPL])
 {
-    if (io.mode == 0) {
+    if (MODE == 0) {
         load_row<PPL>(a, i0, n, vec, v);
         return;
     }
     const int64_t i = min(i0, n - 1);
-    v[0] = a[i];
-    if (io.mode == 1)
-        v[PPL - 1] = b[i];
-    else
-        v[PPL - 1] = b ? __dadd_rn(v[0], __dmul_rn(io.sigma, b[i])) : v[0];
+    const double va = a[i], vb = b[i];
+    v[0] = va;
+    v[PPL - 1] = MODE == 1 ? vb : __dadd_rn(va, __dmul_rn(sigma, vb));
 }
-// output rows: mode 0 -> a; mode 1: v[0] -> a, v[1] -> b; mode 2: v[0] -> a (if given), (v[1] - v[0]) / sigma -> b
-template <int PPL>
+// output rows: MODE 0 -> a; MODE 1: v[0] -> a, v[1] -> b; MODE 2: v[0] -> a (if given), (v[1] - v[0]) (1/sigma) -> b
+template <int PPL, int MODE>
 __device__ __forceinline__ void out_rows(const RatesIO &io, double *__restrict__ a, double *__restrict__ b, int64_t off,
                                          int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
 {
-    if (io.mode == 0) {
+    if (MODE == 0) {
         store_row<PPL>(a + off, i0, n, vec, v);
         return;
     }
     if (i0 >= n) return;
     if (a) a[off + i0] = v[0];
-    b[off + i0] = io.mode == 1 ? v[PPL - 1] : __ddiv_rn(__dsub_rn(v[PPL - 1], v[0]), io.sigma);
+    b[off + i0] = MODE == 1 ? v[PPL - 1] : __dmul_rn(__dsub_rn(v[PPL - 1], v[0]), io.inv_sigma);
 }
 
 // ---- bulk copy global -> shared with mbarrier completion (TMA, non-tensor form) ------------------------------------
@@ -409,7 +407,9 @@ __device__ __forceinline__ double nasa_eval(const double2 *set, double Tu, doubl
     return fma(c45.y, rTu, v);
 }
 
-template <int W, int PPL, int MAXOWN, bool TM>
+// MODE 0: crf_production_rates; 1, 2: the pair / difference-quotient calls (RatesIO.mode); 3: mode 0 with the by-products
+// of crf_rhs_pointwise.  Separate instances: the code of one call does not cost another a register or a branch.
+template <int W, int PPL, int MAXOWN, bool TM, int MODE>
 __global__ void __launch_bounds__(32 * W, 16 / W)
     rates_group_kernel(DevTables m, RatesIO io, int64_t n)
 {
@@ -453,19 +453,20 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
 
     // mode 0: the lane's PPL points are adjacent grid points; modes 1, 2 (PPL = 2): the lane's two "points" are the two
     // states of ONE grid point, so tables, records and lists are read once for both evaluations
-    const int mode = io.mode;
+    constexpr int mode = MODE == 3 ? 0 : MODE;
+    constexpr bool EXT = MODE == 3;
     const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * (mode == 0 ? PPL : 1);
     const bool vec = (n & 1) == 0;
     Ctx<PPL> c;
     double pi[PPL];
-    in_row<PPL>(io, io.T, io.T2, i0, n, vec, c.T);
-    in_row<PPL>(io, io.p, io.p2, i0, n, vec, pi);
+    in_row<PPL, mode>(io, io.T, io.T2, io.sigma, i0, n, vec, c.T);
+    in_row<PPL, mode>(io, io.p, io.p2, io.sigma_p, i0, n, vec, pi);
     // ---- a1: Z_k = Y_k / W_k; warp w takes species w, w + W, ...: all row loads of the warp are in flight together
     double z[MAXOWN][PPL];
 #pragma unroll
     for (int s = 0; s < MAXOWN; ++s) {
         const int k = warp + W * s;
-        if (k < Ns) in_row<PPL>(io, io.Y + (int64_t)k * n, io.Y2 ? io.Y2 + (int64_t)k * n : nullptr, i0, n, vec, z[s]);
+        if (k < Ns) in_row<PPL, mode>(io, io.Y + (int64_t)k * n, io.Y2 + (int64_t)k * n, io.sigma, i0, n, vec, z[s]);
     }
     double lc02[PPL], omL[PPL];
 #pragma unroll
@@ -507,7 +508,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
         rho[u] = pi[u] / (CRF_R_GAS * c.T[u] * s);
         invW[u] = s;
     }
-    if (warp == 0 && mode == 0 && (io.rho || io.Wbar)) {  // by-products of crf_rhs_pointwise (Eq. 1d)
+    if (EXT && warp == 0 && mode == 0 && (io.rho || io.Wbar)) {  // by-products of crf_rhs_pointwise (Eq. 1d)
         double wb[PPL];
 #pragma unroll
         for (int u = 0; u < PPL; ++u) wb[u] = 1.0 / invW[u];
@@ -604,7 +605,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     // ---- store omega; a9: qdot = -sum_k h_k omega_k
     mbar_wait(&mbar[nch & 1], (unsigned)((nch >> 1) + (nch & 1)) & 1u);
     const double2 *sH = reinterpret_cast<const double2 *>(sStage + (size_t)(nch & 1) * sb);
-    const bool emit = mode == 0 && (io.cp || io.h || io.cpk);
+    const bool emit = EXT && mode == 0 && (io.cp || io.h || io.cpk);
     double qd[PPL], cpm[PPL], hm[PPL];
 #pragma unroll
     for (int u = 0; u < PPL; ++u) qd[u] = cpm[u] = hm[u] = 0.0;
@@ -620,7 +621,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
                 hk[u] = nasa_eval<false>(h, c.T[u], c.rT[u], 0.0, Tmid);
                 qd[u] = fma(-hk[u], om[s][u], qd[u]);
             }
-            out_rows<PPL>(io, io.omega, io.omega2, (int64_t)k * n, i0, n, vec, om[s]);
+            out_rows<PPL, mode>(io, io.omega, io.omega2, (int64_t)k * n, i0, n, vec, om[s]);
             if (emit) {
                 // crf_rhs_pointwise: c_pk/R from the h/(RT) set (a_i = (i + 1) c_i), mixture c_p and h; the Y row is
                 // read again (it was consumed by the species this warp handled in the prologue, not the ones it owns)
@@ -663,7 +664,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
             for (int w = 0; w < W; ++w) s += sred[(w * PPL + u) * 32 + lane];
             out[u] = s * (CRF_R_GAS * c.T[u]);
         }
-        out_rows<PPL>(io, io.qdot, io.qdot2, 0, i0, n, vec, out);
+        out_rows<PPL, mode>(io, io.qdot, io.qdot2, 0, i0, n, vec, out);
         if (TM)
             asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(sTmBase), "r"((unsigned)rg.tm_cols)
                          : "memory");
@@ -690,11 +691,18 @@ template <int W, int PPL, int MAXOWN, bool TM>
 cudaError_t launch_k(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
 {
     const size_t smem = rates_group_dynamic_smem(m);
-    cudaError_t e = cudaFuncSetAttribute(rates_group_kernel<W, PPL, MAXOWN, TM>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const bool emit = io.cp || io.h || io.cpk || io.rho || io.Wbar;
+    void (*kernel)(DevTables, RatesIO, int64_t) = rates_group_kernel<W, PPL, MAXOWN, TM, 0>;
+    if (io.mode == 0 && emit) kernel = rates_group_kernel<W, PPL, MAXOWN, TM, 3>;
+    if (io.mode != 0) {
+        if (PPL != 2) return cudaErrorInvalidValue;
+        // (instantiated for two points per lane only)
+        kernel = io.mode == 1 ? rates_group_kernel<W, 2, MAXOWN, TM, 1> : rates_group_kernel<W, 2, MAXOWN, TM, 2>;
+    }
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int64_t per_block = io.mode == 0 ? 32 * PPL : 32;
-    rates_group_kernel<W, PPL, MAXOWN, TM><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, io, n);
+    kernel<<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, io, n);
     crf_count_launch();
     return cudaGetLastError();
 }
