@@ -177,6 +177,20 @@ int crf_production_rates_jv(const crf_mech *mech, const double *T, const double 
                             const double *dp, const double *dY, double sigma, int64_t n, double *omega, double *qdot,
                             double *Jomega, double *Jqdot);
 
+/* The element-local spectral-element diffusion operator on what crf_rhs_pointwise emits: "diffusion"
+ * is the most expensive kernel of the paper's right-hand side.  The fields live on nel hexahedral
+ * elements of polynomial order 7: n = 512 nel points, node (i, j, k) of element e at
+ * 512 e + i + 8 j + 64 k (i along x fastest) = the 8 x 8 x 8 Gauss-Lobatto-Legendre points of the element, which is an
+ * affine box of edge lengths h3[3 e + 0..2] = (hx, hy, hz) [m] (h3: device pointer, nel x 3).  With
+ *   X_k = Y_k Wbar / W_k,   f_k = (W_k / Wbar) (rho D_k) grad X_k,   j_k = -f_k + Y_k sum_j f_j
+ * (j_k = rho Y_k V_k of Eq. 2 with the correction velocity V_c, written without the division by X_k)
+ *   dY[Ns*n]  dY_k[i] = sum_q w_q |J| grad phi_i(x_q) . j_k(x_q)               weak form of -div(rho Y_k V_k), Eq. 1a
+ *   dT[n]     dT[i]   = -sum_q w_q |J| grad phi_i(x_q) . (lambda grad T)(x_q)   weak form of div(lambda grad T), Eq. 1b
+ * with the nodal basis phi_i and GLL quadrature, element by element: no gather-scatter across elements, no boundary
+ * terms and no inverse mass matrix (the assembly steps of the solver).  Units: kg/s and W per node. */
+int crf_sem_diffusion(const crf_mech *mech, const double *h3, const double *T, const double *Wbar, const double *Y,
+                      const double *lambda, const double *rhoD, int64_t nel, double *dY, double *dT);
+
 /* One pass of the whole path with HOST buffers: copies T, p, Y to the device in chunks, runs
  * crf_thermo, crf_production_rates and crf_mix_transport on each chunk and copies the seven
  * outputs back, chunks pipelined over internal streams.  All pointers are host pointers with

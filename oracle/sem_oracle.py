@@ -90,3 +90,32 @@ def sem_diffusion(W, h3, T, Wbar, Y, lam, rhoD, N: int = 8):
     gx, gy, gz = _grad(D, T, h3)
     dT = -_weak_div(D, w, lam * gx, lam * gy, lam * gz, h3).reshape(-1)
     return dict(dY=dY, dT=dT)
+
+
+def sem_diffusion_scale(W, h3, T, Wbar, Y, lam, rhoD, N: int = 8):
+    """dict(dY [Ns, n], dT [n]): the GROSS sums behind sem_diffusion -- the same contractions with |D_im| and the
+    magnitudes of every factor, i.e. the sum of the absolute values of all the products that cancel in dY and dT.
+    The operator differentiates: where a field is nearly constant over an element its result is a small difference
+    of large terms, so a tolerance relative to the result itself would ask for more digits than the inputs carry;
+    this is the scale the parity tolerance is relative to (the analogue of S_k for omega_k)."""
+    W, h3 = np.asarray(W, dtype=np.float64), np.asarray(h3, dtype=np.float64)
+    nel, ns = h3.shape[0], W.size
+    sh = (nel, N, N, N)
+    T, Wbar, lam = (np.abs(np.asarray(a, dtype=np.float64)).reshape(sh) for a in (T, Wbar, lam))
+    Y = np.abs(np.asarray(Y, dtype=np.float64)).reshape((ns,) + sh)
+    rhoD = np.abs(np.asarray(rhoD, dtype=np.float64)).reshape((ns,) + sh)
+    x, w = gll(N)
+    D = np.abs(deriv_matrix(x))
+    f = []
+    for k in range(ns):
+        gx, gy, gz = _grad(D, Y[k] * Wbar / W[k], h3)
+        c = (W[k] / Wbar) * rhoD[k]
+        f.append((c * gx, c * gy, c * gz))
+    fc = [sum(fk[d] for fk in f) for d in range(3)]
+    dY = np.empty((ns, nel * N ** 3))
+    for k in range(ns):
+        j = [f[k][d] + Y[k] * fc[d] for d in range(3)]
+        dY[k] = _weak_div(D, w, j[0], j[1], j[2], h3).reshape(-1)
+    gx, gy, gz = _grad(D, T, h3)
+    dT = _weak_div(D, w, lam * gx, lam * gy, lam * gz, h3).reshape(-1)
+    return dict(dY=dY, dT=dT)

@@ -20,7 +20,7 @@ _lib = None
 EXPORTS = ("crf_mech_create", "crf_mech_destroy", "crf_mech_set_stream", "crf_mech_num_species",
            "crf_mech_num_reactions", "crf_thermo", "crf_thermo_species", "crf_production_rates",
            "crf_mix_transport", "crf_rhs_pointwise", "crf_production_rates_pair", "crf_production_rates_jv",
-           "crf_step_host", "crf_last_error")
+           "crf_sem_diffusion", "crf_step_host", "crf_last_error")
 EXPORTS_DIAG = ("crf_mech_create_ex", "crf_mech_plan_info", "crf_fp64_probe", "crf_launch_count",
                 "crf_transport_schedule")
 
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
         L.crf_rhs_pointwise.argtypes = [vp, dp, dp, dp, i64] + [dp] * 10
         L.crf_production_rates_pair.argtypes = [vp] + [dp] * 6 + [i64] + [dp] * 4
         L.crf_production_rates_jv.argtypes = [vp] + [dp] * 6 + [C.c_double, i64] + [dp] * 4
+        L.crf_sem_diffusion.argtypes = [vp] + [dp] * 6 + [i64, dp, dp]
         L.crf_step_host.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
         L.crf_fp64_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.crf_launch_count.restype = C.c_int64
@@ -226,6 +227,17 @@ class Mechanism:
             _dev(dY, (self.Ns, n)), float(sigma), n, _dev(out[0]), _dev(out[1]), _dev(out[2], (self.Ns, n)),
             _dev(out[3], (n,))))
         return out
+
+    def sem_diffusion(self, h3, T, Wbar, Y, lam, rhoD, dY=None, dT=None):
+        """``crf_sem_diffusion``: (dY [Ns, n], dT [n]) on nel = h3.shape[0] order-7 elements, n = 512 nel."""
+        nel = h3.shape[0]
+        n = 512 * nel
+        dY = torch.empty_like(Y) if dY is None else dY
+        dT = torch.empty_like(T) if dT is None else dT
+        self._sync_stream()
+        _check(lib().crf_sem_diffusion(self._h, _dev(h3, (nel, 3)), _dev(T, (n,)), _dev(Wbar, (n,)), _dev(Y, (self.Ns, n)),
+                                       _dev(lam, (n,)), _dev(rhoD, (self.Ns, n)), nel, _dev(dY, (self.Ns, n)), _dev(dT, (n,))))
+        return dY, dT
 
     def step_host(self, T, p, Y, out: dict | None = None) -> dict:
         """Whole path with HOST tensors (pinned for full bandwidth); returns host tensors."""

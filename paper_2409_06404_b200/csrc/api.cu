@@ -430,6 +430,21 @@ int crf_rhs_pointwise(const crf_mech *mech, const double *T, const double *p, co
     return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_rhs_pointwise");
 }
 
+int crf_sem_diffusion(const crf_mech *mech, const double *h3, const double *T, const double *Wbar, const double *Y,
+                      const double *lambda, const double *rhoD, int64_t nel, double *dY, double *dT)
+{
+    if (!mech) return fail(CRF_EINVAL, "crf_sem_diffusion: null mechanism");
+    if (nel < 0) return fail(CRF_EINVAL, "crf_sem_diffusion: negative element count");
+    if (nel == 0) return CRF_OK;
+    if (nel > (int64_t)1 << 31) return fail(CRF_EINVAL, "crf_sem_diffusion: too many elements");
+    if (!h3 || !T || !Wbar || !Y || !lambda || !rhoD || !dY || !dT) return fail(CRF_EINVAL, "crf_sem_diffusion: null pointer");
+    for (const void *q : {(const void *)h3, (const void *)T, (const void *)Wbar, (const void *)Y, (const void *)lambda,
+                          (const void *)rhoD, (const void *)dY, (const void *)dT})
+        if (misaligned(q)) return fail(CRF_EINVAL, "crf_sem_diffusion: pointers must be 16-byte aligned");
+    cudaError_t e = launch_sem_diffusion(mech->dev, h3, T, Wbar, Y, lambda, rhoD, nel, dY, dT, mech->stream);
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_sem_diffusion");
+}
+
 // Chunked host pipeline: slot s owns a stream and one device buffer holding, for a chunk of c points,
 // T, p, Y[Ns], cp, h, qdot, mu, lambda, omega[Ns], rhoD[Ns] (each row c doubles).
 int crf_step_host(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *cp, double *h,

@@ -132,3 +132,16 @@ def test_heat_operator_is_symmetric_and_negative():
     u, v = rng.standard_normal(n), rng.standard_normal(n)
     assert abs(u @ A(v) - v @ A(u)) <= 1e-12 * abs(u @ A(v))
     assert u @ A(u) < 0.0 and np.abs(A(np.ones(n))).max() <= 1e-12 * np.abs(A(u)).max()
+
+
+def test_gross_scale_bounds_the_result():
+    """sem_diffusion_scale sums the magnitudes of the products sem_diffusion sums: it bounds the result entry by entry,
+    and for a field that is constant over the element (the result is exactly a rounding residue) it stays at the size
+    of the cancelling terms."""
+    rng = np.random.default_rng(21)
+    f = _fields(rng, 2, 3, 8)
+    r, s = so.sem_diffusion(**f), so.sem_diffusion_scale(**f)
+    assert np.all(np.abs(r["dY"]) <= s["dY"] * (1 + 1e-12)) and np.all(np.abs(r["dT"]) <= s["dT"] * (1 + 1e-12))
+    f["T"] = np.full_like(f["T"], 1234.5)
+    r, s = so.sem_diffusion(**f), so.sem_diffusion_scale(**f)
+    assert np.abs(r["dT"]).max() <= 1e-13 * s["dT"].max() and s["dT"].min() > 0.0
