@@ -109,4 +109,53 @@ __device__ __forceinline__ double rcp_newton(double x)
 
 constexpr double kLog2e = 1.4426950408889634074;
 
+// ---- the transcendentals of the production-rates kernels (rates_group.cu, rates_smem.cu, rates_staged.cu) -------------
+// Coefficients in constant memory: the FP64 instructions take them as constant-bank operands instead of occupying (and
+// re-materialising) registers.  (static: every translation unit that includes this header gets its own copy)
+// 2^f on [-1/2, 1/2]: degree 8 (Chebyshev-node interpolant, relative error 1.06e-12) and degree 9 (1.9e-14)
+static __constant__ double kExp2P8[9] = {0x1.0000000000000p+0,  0x1.62e42fef84cf0p-1,  0x1.ebfbdff823cedp-3,
+                                         0x1.c6b08dd6fd234p-5,  0x1.3b2ab7181b755p-7,  0x1.5d8745a728441p-10,
+                                         0x1.4308ac85aa947p-13, 0x1.00dc4a532fb8ep-16, 0x1.63d136366db24p-20};
+static __constant__ double kExp2P9[10] = {0x1.000000000003dp+0,  0x1.62e42fefa39f7p-1,  0x1.ebfbdff8149f2p-3,
+                                          0x1.c6b08d7044119p-5,  0x1.3b2ab72b175eep-7,  0x1.5d87fe908f88ap-10,
+                                          0x1.43088e257f341p-13, 0x1.ffcb76789860fp-17, 0x1.63ef969a64d3cp-20,
+                                          0x1.b6571de2f2351p-24};
+static __constant__ double kAtanhOdd[9] = {1.0,        1.0 / 3.0,  1.0 / 5.0,  1.0 / 7.0, 1.0 / 9.0,
+                                           1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0, 1.0 / 17.0};
+
+// 2^y by the degree-DEG polynomial (8 or 9), the exponent clamped from below: an underflowing rate constant becomes a
+// negligible number instead of wrapping into the sign bit.  |y| < 2^31 (callers clamp arguments that can be
+// arbitrarily large before the range reduction).
+template <int DEG>
+__device__ __forceinline__ double exp2_clamped(double y)
+{
+    static_assert(DEG == 8 || DEG == 9, "degree 8 or 9");
+    const double magic = 6755399441055744.0;  // 1.5 * 2^52
+    const double t = __dadd_rn(y, magic);
+    const int k = max(__double2loint(t), -1000);
+    const double f = __dsub_rn(y, __dsub_rn(t, magic));
+    double p = DEG == 8 ? kExp2P8[8] : kExp2P9[9];
+#pragma unroll
+    for (int i = DEG - 1; i >= 0; --i) p = fma(p, f, DEG == 8 ? kExp2P8[i] : kExp2P9[i]);
+    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+// log2(x) for normal x > 0, branch-free: x = 2^e m, m in [sqrt(1/2), sqrt(2)), ln m = 2 atanh((m-1)/(m+1)), the odd
+// series truncated after TERMS terms (|s| <= 0.172: 7 terms = absolute error 2e-12, 9 terms = 3e-15)
+template <int TERMS>
+__device__ __forceinline__ double log2_atanh(double x)
+{
+    static_assert(TERMS >= 2 && TERMS <= 9, "2..9 terms");
+    int hi = __double2hiint(x);
+    const int e = (hi - 0x3fe6a09e) >> 20;
+    hi -= e << 20;
+    const double m = __hiloint2double(hi, __double2loint(x));
+    const double s = (m - 1.0) * rcp_newton(m + 1.0);
+    const double z = s * s;
+    double p = kAtanhOdd[TERMS - 1];
+#pragma unroll
+    for (int i = TERMS - 2; i >= 0; --i) p = fma(p, z, kAtanhOdd[i]);
+    return fma(s * (2.0 * kLog2e), p, (double)e);
+}
+
 }  // namespace crf

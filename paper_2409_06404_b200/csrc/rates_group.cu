@@ -37,51 +37,10 @@
 
 namespace {
 
-// 2^f on [-1/2, 1/2], degree 8 (Chebyshev-node interpolant, relative error 1.06e-12), and the odd atanh series, in
-// constant memory: the FP64 instructions take the coefficients as constant-bank operands
-__constant__ double kExp2[9] = {0x1.0000000000000p+0,  0x1.62e42fef84cf0p-1,  0x1.ebfbdff823cedp-3,
-                                0x1.c6b08dd6fd234p-5,  0x1.3b2ab7181b755p-7,  0x1.5d8745a728441p-10,
-                                0x1.4308ac85aa947p-13, 0x1.00dc4a532fb8ep-16, 0x1.63d136366db24p-20};
-__constant__ double kAtanh[7] = {1.0, 1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0};
-
-// 2^y; the exponent is clamped from below: an underflowing rate constant becomes a negligible number instead of
-// wrapping into the sign bit.  |y| < 2^31 (callers clamp arguments that can be arbitrarily large).
-__device__ __forceinline__ double exp2r(double y)
-{
-    const double magic = 6755399441055744.0;  // 1.5 * 2^52
-    const double t = __dadd_rn(y, magic);
-    const int k = max(__double2loint(t), -1000);
-    const double f = __dsub_rn(y, __dsub_rn(t, magic));
-    double p = kExp2[8];
-#pragma unroll
-    for (int i = 7; i >= 0; --i) p = fma(p, f, kExp2[i]);
-    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
-}
-
-// 1/x for normal x: MUFU.RCP64H seed (relative error < 2^-20) and one cubic Newton step
-__device__ __forceinline__ double rcp_fast(double x)
-{
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double e = fma(-x, y, 1.0);
-    return fma(y, fma(e, e, e), y);
-}
-
-// log2(x) for normal x > 0, branch-free: x = 2^e m, m in [sqrt(1/2), sqrt(2)), ln m = 2 atanh((m-1)/(m+1));
-// series truncated after s^13 (|s| <= 0.172: absolute error 2e-12)
-__device__ __forceinline__ double log2_fast(double x)
-{
-    int hi = __double2hiint(x);
-    const int e = (hi - 0x3fe6a09e) >> 20;
-    hi -= e << 20;
-    const double m = __hiloint2double(hi, __double2loint(x));
-    const double s = (m - 1.0) * rcp_fast(m + 1.0);
-    const double z = s * s;
-    double p = kAtanh[6];
-#pragma unroll
-    for (int i = 5; i >= 0; --i) p = fma(p, z, kAtanh[i]);
-    return fma(s * (2.0 * crf::kLog2e), p, (double)e);
-}
+// the transcendentals (fastmath.cuh): 2^y by the degree-8 polynomial (1.1e-12), Newton reciprocal, atanh-series log2
+__device__ __forceinline__ double exp2r(double y) { return crf::exp2_clamped<8>(y); }
+__device__ __forceinline__ double rcp_fast(double x) { return crf::rcp_newton(x); }
+__device__ __forceinline__ double log2_fast(double x) { return crf::log2_atanh<7>(x); }
 
 // ---- rows: [lane][PPL] doubles; a lane's PPL points are adjacent -------------------------------------------------
 template <int PPL>

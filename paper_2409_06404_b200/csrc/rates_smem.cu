@@ -21,50 +21,10 @@
 
 namespace {
 
-// 2^f on [-1/2, 1/2], degree 9 (fastmath.cuh), in constant memory: the FP64 instructions take the
-// coefficients as constant-bank operands instead of occupying (and re-materialising) registers
-__constant__ double kExp2[10] = {0x1.000000000003dp+0, 0x1.62e42fefa39f7p-1,  0x1.ebfbdff8149f2p-3, 0x1.c6b08d7044119p-5,
-                                 0x1.3b2ab72b175eep-7, 0x1.5d87fe908f88ap-10, 0x1.43088e257f341p-13, 0x1.ffcb76789860fp-17,
-                                 0x1.63ef969a64d3cp-20, 0x1.b6571de2f2351p-24};
-__constant__ double kAtanh[9] = {1.0, 1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0, 1.0 / 17.0};
-
-__device__ __forceinline__ double exp2c(double y)
-{
-    // crf::exp2_poly9 with the exponent clamped from below: an underflowing rate constant becomes a
-    // negligible number instead of wrapping into the sign bit
-    const double magic = 6755399441055744.0;
-    const double t = __dadd_rn(y, magic);
-    const int k = max(__double2loint(t), -1000);
-    const double f = __dsub_rn(y, __dsub_rn(t, magic));
-    double p = kExp2[9];
-#pragma unroll
-    for (int i = 8; i >= 0; --i) p = fma(p, f, kExp2[i]);
-    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
-}
-
-// 1/x for normal x: MUFU.RCP64H seed (relative error < 2^-20) and one cubic Newton step
-__device__ __forceinline__ double rcp_fast(double x)
-{
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double e = fma(-x, y, 1.0);
-    return fma(y, fma(e, e, e), y);
-}
-
-// log2(x) for normal x > 0, branch-free: x = 2^e m, m in [sqrt(1/2), sqrt(2)), ln m = 2 atanh((m-1)/(m+1))
-__device__ __forceinline__ double log2_fast(double x)
-{
-    int hi = __double2hiint(x);
-    const int e = (hi - 0x3fe6a09e) >> 20;
-    hi -= e << 20;
-    const double m = __hiloint2double(hi, __double2loint(x));
-    const double s = (m - 1.0) * rcp_fast(m + 1.0);
-    const double z = s * s;
-    double p = kAtanh[8];
-#pragma unroll
-    for (int i = 7; i >= 0; --i) p = fma(p, z, kAtanh[i]);
-    return fma(s * (2.0 * crf::kLog2e), p, (double)e);
-}
+// the transcendentals (fastmath.cuh): 2^y by the degree-9 polynomial, Newton reciprocal, atanh-series log2 (9 terms)
+__device__ __forceinline__ double exp2c(double y) { return crf::exp2_clamped<9>(y); }
+__device__ __forceinline__ double rcp_fast(double x) { return crf::rcp_newton(x); }
+__device__ __forceinline__ double log2_fast(double x) { return crf::log2_atanh<9>(x); }
 
 template <int PPL>
 struct Ctx {

@@ -25,26 +25,7 @@
 
 namespace {
 
-__device__ __forceinline__ double exp2_clamped(double y)
-{
-    // as crf::exp2_poly9, with the exponent clamped from below so that an underflowing rate constant
-    // becomes a negligible number instead of wrapping into the sign bit
-    const double magic = 6755399441055744.0;
-    const double t = __dadd_rn(y, magic);
-    const int k = max(__double2loint(t), -1000);
-    const double f = __dsub_rn(y, __dsub_rn(t, magic));
-    double p = 0x1.b6571de2f2351p-24;
-    p = fma(p, f, 0x1.63ef969a64d3cp-20);
-    p = fma(p, f, 0x1.ffcb76789860fp-17);
-    p = fma(p, f, 0x1.43088e257f341p-13);
-    p = fma(p, f, 0x1.5d87fe908f88ap-10);
-    p = fma(p, f, 0x1.3b2ab72b175eep-7);
-    p = fma(p, f, 0x1.c6b08d7044119p-5);
-    p = fma(p, f, 0x1.ebfbdff8149f2p-3);
-    p = fma(p, f, 0x1.62e42fefa39f7p-1);
-    p = fma(p, f, 0x1.000000000003dp+0);
-    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
-}
+__device__ __forceinline__ double exp2_clamped(double y) { return crf::exp2_clamped<9>(y); }  // (fastmath.cuh)
 
 struct PointCtx {
     double L, rT, lc02;  // ln T, 1/T, log2(e) ln(p_ref/(R T))
