@@ -41,9 +41,10 @@ def parse():
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--points", type=int, default=0, help="override the number of points (debug)")
     ap.add_argument("--cpu-points", type=int, default=0, help="oracle sample size (default: ~10-30 s of CPU)")
-    ap.add_argument("--path", default="three", choices=["three", "rhs", "jv"],
+    ap.add_argument("--path", default="three", choices=["three", "rhs", "jv", "sem"],
                     help="three: crf_thermo + crf_production_rates + crf_mix_transport (the default step); rhs: one "
-                         "crf_rhs_pointwise call (SURVEY 8(f)1); jv: one crf_production_rates_jv call (8(f)2)")
+                         "crf_rhs_pointwise call (SURVEY 8(f)1); jv: one crf_production_rates_jv call (8(f)2); sem: one "
+                         "crf_sem_diffusion call on the outputs of crf_rhs_pointwise (8(f)3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -54,7 +55,7 @@ CPU_SAMPLE = {"C1": 512, "C2": 1 << 20, "C3": 1 << 19, "C4": 1 << 18, "C5": 1 <<
 
 
 CALLS = {"three": ["crf_thermo", "crf_production_rates", "crf_mix_transport"], "rhs": ["crf_rhs_pointwise"],
-         "jv": ["crf_production_rates_jv"]}
+         "jv": ["crf_production_rates_jv"], "sem": ["crf_sem_diffusion"]}
 
 
 def config_dict(name, n, world, path="three"):
@@ -226,6 +227,27 @@ def other_path(args, mech, dev, out, n, name, world, rank, local, barrier, flush
         flops = w_th["F"] + w_ra["F"] + w_tr["F"]
         alg_bytes = 8 * (Ns + 2) + 8 * (3 * Ns + 7)  # one read of T, p, Y; omega, rhoD, c_pk rows and 7 scalar fields
         sep_name, sep_note = "three_calls", "crf_thermo + crf_production_rates + crf_mix_transport (no rho, Wbar, c_pk)"
+    elif args.path == "sem":
+        rhs = mech.rhs_pointwise(dev["T"], dev["p"], dev["Y"], want_cpk=False)
+        nel = n // 512
+        h3 = torch.from_numpy(np.random.default_rng(7 + rank).uniform(0.2e-3, 1.5e-3, (nel, 3))).cuda()
+        dYo, dTo = torch.empty(Ns, n, **f64), torch.empty(n, **f64)
+        gY = torch.empty(3, n, **f64)
+
+        def fused():
+            mech.sem_diffusion(h3, dev["T"], rhs["Wbar"], dev["Y"], rhs["lam"], rhs["rhoD"], dYo, dTo)
+
+        def separate():  # the pure stream of the same bytes: what a copy kernel needs for this operator's traffic
+            dYo.copy_(dev["Y"])
+            out["omega"].copy_(rhs["rhoD"])
+            dTo.copy_(dev["T"])
+            gY[0].copy_(rhs["lam"])
+            gY[1].copy_(rhs["Wbar"])
+        # algorithmic minimum per node and field: 24 FMA for the gradient (ONCE: the kernel's second evaluation in pass 2 is
+        # its own choice, not the method's), 24 for the weak divergence, ~20 pointwise
+        flops = 2 * ((24 + 24 + 20) * Ns + 24 + 24 + 10)
+        alg_bytes = 8 * (3 * Ns + 4)  # Y, rho D in, dY out; T, lambda, Wbar in, dT out
+        sep_name, sep_note = "copy_calls", "torch copies of the operator's algorithmic bytes (3 Ns + 4 fields in + out): the HBM stream it is bounded by"
     else:
         gen = torch.Generator(device="cuda").manual_seed(1234 + rank)
         v = {k: dev[k] * (2 * torch.rand(dev[k].shape, generator=gen, **f64) - 1) for k in ("T", "p", "Y")}
@@ -283,8 +305,11 @@ def other_path(args, mech, dev, out, n, name, world, rank, local, barrier, flush
     t_alu = flops * n / (rooflines.FP64_PEAK_TFLOPS * 1e12)
     t_hbm = alg_bytes * n / (peaks["hbm_gbs"] * 1e9)
     call = CALLS[args.path][0]
-    roof = {"bound": "alu" if t_alu >= t_hbm else "hbm", "kernel": call, "achieved": flops * n / (ms * 1e-3) / 1e12,
-            "peak": rooflines.FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": max(t_alu, t_hbm) / (ms * 1e-3), "traffic": None,
+    hbm_bound = t_hbm > t_alu
+    roof = {"bound": "hbm" if hbm_bound else "alu", "kernel": call,
+            "achieved": alg_bytes * n / (ms * 1e-3) / 1e9 if hbm_bound else flops * n / (ms * 1e-3) / 1e12,
+            "peak": peaks["hbm_gbs"] if hbm_bound else rooflines.FP64_PEAK_TFLOPS, "unit": "GB/s" if hbm_bound else "TFLOP/s",
+            "frac": max(t_alu, t_hbm) / (ms * 1e-3), "traffic": None,
             "peak_source": "148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md); FMA = 2 flops",
             "flops_per_point": flops, "bytes_per_point": alg_bytes, "t_hbm_ms": 1e3 * t_hbm, "t_alu_ms": 1e3 * t_alu}
     line = {"metric": METRIC, "value": world * n / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
