@@ -181,7 +181,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
                                   : (rgo.W > 0 ? CRF_RATES_GROUP : (rpo.W > 0 ? CRF_RATES_STAGED : CRF_RATES_GENERIC));
     if (rso.W > 0)
         info.rates_W = rso.W, info.rates_PPL = rso.PPL, info.rates_Rc = rso.Rc, info.rates_chunks = rso.n_chunks,
-        info.rates_stage_bytes = rso.stage_bytes;
+        info.rates_stage_bytes = rso.stage_bytes, info.rates_tmem_cols = (opt.rates_tmem != 1 && 6 * (Ns + 1) <= 512) ? 6 * (Ns + 1) : 0;
     else if (rgo.W > 0)
         info.rates_W = rgo.W, info.rates_PPL = rgo.PPL, info.rates_Rc = rgo.Rc, info.rates_chunks = rgo.n_chunks,
         info.rates_stage_bytes = rgo.stage_bytes, info.rates_tmem_cols = rgo.tm_cols;
@@ -238,6 +238,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
     rp.inc = reinterpret_cast<const double2 *>(base + rpo.inc);
     rp.troe = D(rpo.troe), rp.gco = D(rpo.gco), rp.hco = D(rpo.hco);
     RatesSmemPlan &rs = d.rs;
+    rs.tmem = (opt.rates_tmem != 1 && 6 * (Ns + 1) <= 512) ? 1 : 0;
     rs.W = rso.W, rs.PPL = rso.PPL, rs.maxown = rso.maxown, rs.Rc = rso.Rc, rs.n_chunks = rso.n_chunks, rs.stage_bytes = rso.stage_bytes;
     rs.chunk = reinterpret_cast<const int4 *>(base + rso.chunk);
     rs.stage = base + rso.stage;
@@ -367,9 +368,11 @@ int crf_production_rates_pair(const crf_mech *mech, const double *T, const doubl
                           (const void *)Y2, (const void *)omega, (const void *)qdot, (const void *)omega2, (const void *)qdot2})
         if (misaligned(q)) return fail(CRF_EINVAL, "crf_production_rates_pair: pointers must be 16-byte aligned");
     cudaError_t e;
-    if (mech->dev.rg.W > 0 && mech->dev.rg.PPL == 2) {
-        RatesIO io = rates_io(T, p, Y, omega, qdot);
-        io.T2 = T2, io.p2 = p2, io.Y2 = Y2, io.omega2 = omega2, io.qdot2 = qdot2, io.mode = 1;
+    RatesIO io = rates_io(T, p, Y, omega, qdot);
+    io.T2 = T2, io.p2 = p2, io.Y2 = Y2, io.omega2 = omega2, io.qdot2 = qdot2, io.mode = 1;
+    if (rates_thread_tm_serves(mech->dev, io)) {  // (small mechanisms: the thread kernel evaluates both states per launch)
+        e = launch_rates_thread_io(mech->dev, io, n, mech->stream);
+    } else if (mech->dev.rg.W > 0 && mech->dev.rg.PPL == 2) {
         e = launch_rates_group(mech->dev, io, n, mech->stream);
     } else {  // no plan that shares a launch: two launches of whatever kernel the mechanism runs
         e = launch_rates(mech->dev, T, p, Y, n, omega, qdot, mech->stream);
@@ -390,13 +393,17 @@ int crf_production_rates_jv(const crf_mech *mech, const double *T, const double 
     for (const void *q : {(const void *)T, (const void *)p, (const void *)Y, (const void *)dT, (const void *)dp,
                           (const void *)dY, (const void *)omega, (const void *)qdot, (const void *)Jomega, (const void *)Jqdot})
         if (misaligned(q)) return fail(CRF_EINVAL, "crf_production_rates_jv: pointers must be 16-byte aligned");
-    if (!(mech->dev.rg.W > 0 && mech->dev.rg.PPL == 2))
-        return fail(CRF_EUNSUPPORTED, "crf_production_rates_jv: this mechanism has no warp-group plan with two states per lane "
-                                      "(use crf_production_rates_pair on a perturbed copy)");
     RatesIO io = rates_io(T, p, Y, omega, qdot);
     io.T2 = dT, io.Y2 = dY, io.omega2 = Jomega, io.qdot2 = Jqdot, io.sigma = sigma, io.inv_sigma = 1.0 / sigma, io.mode = 2;
     io.p2 = dp ? dp : p, io.sigma_p = dp ? sigma : 0.0;  // (no pressure perturbation: p + 0 p)
-    cudaError_t e = launch_rates_group(mech->dev, io, n, mech->stream);
+    cudaError_t e;
+    if (rates_thread_tm_serves(mech->dev, io))
+        e = launch_rates_thread_io(mech->dev, io, n, mech->stream);
+    else if (mech->dev.rg.W > 0 && mech->dev.rg.PPL == 2)
+        e = launch_rates_group(mech->dev, io, n, mech->stream);
+    else
+        return fail(CRF_EUNSUPPORTED, "crf_production_rates_jv: this mechanism has no warp-group plan with two states per lane "
+                                      "(use crf_production_rates_pair on a perturbed copy)");
     return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_production_rates_jv");
 }
 
@@ -414,11 +421,13 @@ int crf_rhs_pointwise(const crf_mech *mech, const double *T, const double *p, co
     const DevTables &d = mech->dev;
     cudaStream_t st = mech->stream;
     cudaError_t e;
-    if (d.rg.W > 0) {
+    RatesIO io = rates_io(T, p, Y, omega, qdot);
+    io.cp = cp, io.h = h, io.cpk = cpk, io.rho = rho, io.Wbar = Wbar;
+    if (rates_thread_tm_serves(d, io)) {
+        e = launch_rates_thread_io(d, io, n, st);
+    } else if (d.rg.W > 0) {
         // the thermodynamic by-products leave the production-rates kernel (it evaluates the NASA sets and the
         // composition anyway): no separate thermo pass, Y is read by two kernels instead of three
-        RatesIO io = rates_io(T, p, Y, omega, qdot);
-        io.cp = cp, io.h = h, io.cpk = cpk, io.rho = rho, io.Wbar = Wbar;
         e = launch_rates_group(d, io, n, st);
     } else {
         e = launch_rates(d, T, p, Y, n, omega, qdot, st);

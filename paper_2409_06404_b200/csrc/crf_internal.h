@@ -72,6 +72,7 @@ struct RatesSmemPlan {
     int Rc;           // q buffer rows (max reactions per chunk)
     int n_chunks;
     int stage_bytes;  // largest chunk block, multiple of 16
+    int tmem;         // thread kernel: the per-thread state lives in tensor memory (6 (Ns + 1) <= 512 columns)
     const int4 *chunk;           // [n_chunks]: x = kind (0 elementary, 1 third body, 2 falloff) | generic << 2,
                                  //   y = reactions, z = byte offset of the block in stage, w = block bytes
     const unsigned char *stage;

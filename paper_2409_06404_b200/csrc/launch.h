@@ -45,6 +45,8 @@ cudaError_t launch_rates_staged(const DevTables &m, const double *T, const doubl
 cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n,
                               double *omega, double *qdot, cudaStream_t st);
 cudaError_t launch_rates_group(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st);
+bool rates_thread_tm_serves(const DevTables &m, const RatesIO &io);
+cudaError_t launch_rates_thread_io(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st);
 cudaError_t launch_sem_diffusion(const DevTables &m, const double *h3, const double *T, const double *Wbar, const double *Y,
                                  const double *lam, const double *rhoD, int64_t nel, double *dY, double *dT, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *inst_per_s);

@@ -205,7 +205,7 @@ RatesSmemPlanOffsets build_rates_smem_plan(const crf_tables *t, const crf_plan_o
             g[4] = -s * A(4) / 20.0, g[5] = s * A(5), g[6] = -s * A(6);
             h[0] = A(0), h[1] = A(1) / 2.0, h[2] = A(2) / 3.0, h[3] = A(3) / 4.0, h[4] = A(4) / 5.0, h[5] = A(5);
             if (rg == 0) g[7] = t->Tmid[k], h[7] = t->Tmid[k];
-            if (rg == 1) g[7] = 1.0 / t->W[k];
+            if (rg == 1) g[7] = 1.0 / t->W[k], h[7] = 1.0 / t->W[k];
         }
     o.chunk = b.add(cdesc), o.stage = b.add(stage), o.gco = b.add(gco), o.hco = b.add(hco);
     return o;

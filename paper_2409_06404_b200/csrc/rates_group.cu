@@ -34,6 +34,7 @@
 #include "crf_internal.h"
 #include "fastmath.cuh"
 #include "launch.h"
+#include "tmem.cuh"
 
 namespace {
 
@@ -146,49 +147,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
         : "memory");
 }
 
-// ---- tensor memory as per-lane storage: lane = this thread's lane of the warp's quadrant, 32-bit columns ---------------
-// A row of PPL doubles is 2 PPL columns.  Loads are asynchronous: the registers are valid after tm_wait, which takes
-// them as operands so that no use can be scheduled before it.
-template <int PPL>
-struct TmRow {
-    unsigned r[2 * PPL];
-};
-template <int PPL>
-__device__ __forceinline__ void tm_ld(unsigned taddr, TmRow<PPL> &t)
-{
-    if (PPL == 2)
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
-                     : "=r"(t.r[0]), "=r"(t.r[1]), "=r"(t.r[2 * PPL - 2]), "=r"(t.r[2 * PPL - 1])
-                     : "r"(taddr));
-    else
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(t.r[0]), "=r"(t.r[1]) : "r"(taddr));
-}
-template <int PPL>
-__device__ __forceinline__ void tm_st(unsigned taddr, const double (&v)[PPL])
-{
-    if (PPL == 2)
-        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(__double2loint(v[0])),
-                     "r"(__double2hiint(v[0])), "r"(__double2loint(v[PPL - 1])), "r"(__double2hiint(v[PPL - 1]))
-                     : "memory");
-    else
-        asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(__double2loint(v[0])),
-                     "r"(__double2hiint(v[0]))
-                     : "memory");
-}
-template <int PPL>
-__device__ __forceinline__ void tm_wait1(TmRow<PPL> &a)
-{
-    if (PPL == 2)
-        asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(a.r[0]), "+r"(a.r[1]), "+r"(a.r[2 * PPL - 2]), "+r"(a.r[2 * PPL - 1]));
-    else
-        asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(a.r[0]), "+r"(a.r[1]));
-}
-template <int PPL>
-__device__ __forceinline__ void tm_get(const TmRow<PPL> &t, double (&v)[PPL])
-{
-#pragma unroll
-    for (int u = 0; u < PPL; ++u) v[u] = __hiloint2double((int)t.r[2 * u + 1], (int)t.r[2 * u]);
-}
+using crf::TmRow;
+using crf::tm_get;
+using crf::tm_ld;
+using crf::tm_st;
+using crf::tm_wait1;
 
 // the u row of one species: from tensor memory (h = column) or from shared memory (h = byte offset in the state)
 template <bool TM, int PPL>

@@ -15,9 +15,12 @@
 // Reactions are cut into chunks of one kind (elementary | third body | Troe falloff; two or three species per side);
 // all chunk blocks (48-byte reaction records, third-body lists, Troe sets) are resident in shared memory.
 // Troe falloff is evaluated in base 2 (log2 F = log2 F_cent / (1 + f1^2)) with a branch-free logarithm.
+#include <algorithm>
+
 #include "crf_internal.h"
 #include "fastmath.cuh"
 #include "launch.h"
+#include "tmem.cuh"
 
 namespace {
 
@@ -37,9 +40,10 @@ __device__ __forceinline__ uint4 ldsu4(const char *p) { return *reinterpret_cast
 
 // q of one reaction at the PPL points of this lane.  rec: the 48-byte record; tr: its Troe set (kind 2);
 // sL: the (C, d) state at this lane (row offsets come from the record; point u is 512 u bytes further).
-template <int KIND, bool GENERIC, int PPL>
+// TM: the (C, d) pairs live in tensor memory (PPL = 1; tmq = this warp's quadrant address; pair k at column 4 k = row offset / 512).
+template <int KIND, bool GENERIC, int PPL, bool TM = false>
 __device__ __forceinline__ void reaction_q(const char *blk, const char *rec, const char *tr, const char *sL,
-                                           const Ctx<PPL> &c, double (&q)[PPL])
+                                           const Ctx<PPL> &c, double (&q)[PPL], unsigned tmq = 0u)
 {
     const double2 A = lds2(rec);        // log2e lnA, log2e beta
     const double2 Ex = lds2(rec + 16);  // -log2e Ea/R, (x0, x1)
@@ -54,17 +58,45 @@ __device__ __forceinline__ void reaction_q(const char *blk, const char *rec, con
             const uint4 en = ldsu4(e);
             const double coef = __hiloint2double((int)en.y, (int)en.x);
 #pragma unroll
-            for (int u = 0; u < PPL; ++u) M[u] = fma(coef, lds2(sL + en.z + 512 * u).x, M[u]);
+            for (int u = 0; u < PPL; ++u) {
+                double Ck;
+                if (TM) {
+                    crf::TmRow<1> r;
+                    crf::tm_ld<1>(tmq + (en.z >> 9), r);
+                    crf::tm_wait1<1>(r);
+                    Ck = crf::tm_one(r);
+                } else {
+                    Ck = lds2(sL + en.z + 512 * u).x;
+                }
+                M[u] = fma(coef, Ck, M[u]);
+            }
         }
     }
 #pragma unroll
     for (int u = 0; u < PPL; ++u) {
         const char *s = sL + 512 * u;
         const double yinf = fma(A.y, c.L[u], fma(Ex.x, c.rT[u], A.x));  // log2 k_f (high-pressure limit)
-        const double2 a0 = lds2(s + S.x), a1 = lds2(s + S.y), b0 = lds2(s + S.z), b1 = lds2(s + S.w);
+        double2 a0, a1, b0, b1;
+        if (TM) {
+            crf::TmRow<2> r0, r1, r2, r3;
+            crf::tm_ld<2>(tmq + (S.x >> 9), r0), crf::tm_ld<2>(tmq + (S.y >> 9), r1);
+            crf::tm_ld<2>(tmq + (S.z >> 9), r2), crf::tm_ld<2>(tmq + (S.w >> 9), r3);
+            crf::tm_wait4(r0, r1, r2, r3);
+            a0 = crf::tm_pair(r0), a1 = crf::tm_pair(r1), b0 = crf::tm_pair(r2), b1 = crf::tm_pair(r3);
+        } else {
+            a0 = lds2(s + S.x), a1 = lds2(s + S.y), b0 = lds2(s + S.z), b1 = lds2(s + S.w);
+        }
         double Pf = a0.x * a1.x, Pr = b0.x * b1.x, num = a0.y * a1.y, den = b0.y * b1.y;
         if (GENERIC) {
-            const double2 a2 = lds2(s + x0), b2 = lds2(s + x1);
+            double2 a2, b2;
+            if (TM) {
+                crf::TmRow<2> r0, r1;
+                crf::tm_ld<2>(tmq + (x0 >> 9), r0), crf::tm_ld<2>(tmq + (x1 >> 9), r1);
+                crf::tm_wait1<2>(r0), crf::tm_wait1<2>(r1);
+                a2 = crf::tm_pair(r0), b2 = crf::tm_pair(r1);
+            } else {
+                a2 = lds2(s + x0), b2 = lds2(s + x1);
+            }
             Pf *= a2.x, Pr *= b2.x, num *= a2.y, den *= b2.y;
         }
         // 1/K_c = num/den with the MUFU seed and ONE Newton step (relative error 2^-40: the tolerance of omega is
@@ -250,6 +282,258 @@ __global__ void __launch_bounds__(RT_B) rates_thread_kernel(DevTables m, const d
     if (i < n) qdot[i] = qd * (CRF_R_GAS * Tu);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The same kernel with the per-thread state in TENSOR MEMORY (tmem.cuh): the (C, d) pair of species k in columns
+// 4 k .. 4 k + 3 of the thread's lane, omega_k in columns 4 (Ns + 1) + 2 k.  ncu showed the shared-memory version
+// bound by the shared-memory pipe (90 % of its wavefronts on C2): every state access there is a non-broadcast 64- or
+// 128-bit access per lane.  Tensor memory is indexed by a warp-uniform column (the species of the reaction) and has its
+// own data path; shared memory keeps only the mechanism's tables (broadcast reads).
+__device__ __forceinline__ void scatter_q_tm(unsigned tom, const char *rec, double q, bool generic)
+{
+    const uint4 S = ldsu4(rec + 32);  // state row offsets (stride 2048) -> omega columns (2 per species)
+    const unsigned c0 = tom + (S.x >> 10), c1 = tom + (S.y >> 10), c2 = tom + (S.z >> 10), c3 = tom + (S.w >> 10);
+    if (!generic && S.x != S.y && S.z != S.w && S.x != S.z && S.x != S.w && S.y != S.z && S.y != S.w) {
+        // four distinct species (a warp-uniform test): the four loads go out together, then the four stores
+        crf::TmRow<1> r0, r1, r2, r3;
+        crf::tm_ld<1>(c0, r0), crf::tm_ld<1>(c1, r1), crf::tm_ld<1>(c2, r2), crf::tm_ld<1>(c3, r3);
+        crf::tm_wait4(r0, r1, r2, r3);
+        const double v0[1] = {crf::tm_one(r0) - q}, v1[1] = {crf::tm_one(r1) - q}, v2[1] = {crf::tm_one(r2) + q},
+                     v3[1] = {crf::tm_one(r3) + q};
+        crf::tm_st<1>(c0, v0), crf::tm_st<1>(c1, v1), crf::tm_st<1>(c2, v2), crf::tm_st<1>(c3, v3);
+        return;
+    }
+    auto add = [&](unsigned col, double dq) {  // (a species listed twice: the updates must follow one another)
+        crf::TmRow<1> r;
+        crf::tm_ld<1>(col, r);
+        crf::tm_wait1<1>(r);
+        const double v[1] = {crf::tm_one(r) + dq};
+        crf::tm_st<1>(col, v);
+        crf::tm_wait_st();
+    };
+    add(c0, -q), add(c1, -q), add(c2, q), add(c3, q);
+    if (generic) {
+        const uint2 X = *reinterpret_cast<const uint2 *>(rec + 24);
+        add(tom + (X.x >> 10), -q), add(tom + (X.y >> 10), q);
+    }
+}
+
+template <int KIND, bool GENERIC>
+__device__ __forceinline__ void thread_chunk_tm(const char *blk, int count, int o_troe, unsigned tmq, unsigned tom, const Ctx<1> &c)
+{
+    constexpr int NR = 2;  // independent reactions per trip (1, 3, 4 measured: no difference)
+    int rl = 0;
+    for (; rl + NR - 1 < count; rl += NR) {
+        double q[NR][1];
+#pragma unroll
+        for (int v = 0; v < NR; ++v)
+            reaction_q<KIND, GENERIC, 1, true>(blk, blk + 48 * (rl + v), blk + o_troe + 64 * (rl + v), nullptr, c, q[v], tmq);
+#pragma unroll
+        for (int v = 0; v < NR; ++v) {
+            scatter_q_tm(tom, blk + 48 * (rl + v), q[v][0], GENERIC);
+            crf::tm_wait_st();  // (the next reaction may update the same species)
+        }
+    }
+    for (; rl < count; ++rl) {
+        double q0[1];
+        reaction_q<KIND, GENERIC, 1, true>(blk, blk + 48 * rl, blk + o_troe + 64 * rl, nullptr, c, q0, tmq);
+        scatter_q_tm(tom, blk + 48 * rl, q0[0], GENERIC);
+        crf::tm_wait_st();
+    }
+}
+
+// MODE (RatesIO.mode; 3 = mode 0 with the by-products of crf_rhs_pointwise): in modes 1 and 2 the thread evaluates the
+// two states of its grid point one after the other (the tables are staged once; omega of the first state stays in
+// tensor memory until the quotient is formed).
+template <int MODE>
+__global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, RatesIO io, int64_t n, unsigned tm_cols)
+{
+    extern __shared__ double2 sm2[];
+    __shared__ unsigned sTmBase;
+    const RatesSmemPlan &rs = m.rs;
+    const int Ns = m.Ns, tid = threadIdx.x, warp = tid >> 5;
+    char *sTab = reinterpret_cast<char *>(sm2);  // the chunk blocks
+    char *sGH = sTab + rs.stage_bytes;            // g/(RT) sets [Ns][128 B], then h/(RT) sets [Ns][128 B]
+    if (warp == 0) crf::tm_alloc(&sTmBase, tm_cols);
+    for (int o = tid * 16; o < rs.stage_bytes; o += RT_B * 16)
+        *reinterpret_cast<uint4 *>(sTab + o) = __ldg(reinterpret_cast<const uint4 *>(rs.stage + o));
+    for (int o = tid * 16; o < 128 * Ns; o += RT_B * 16) {
+        *reinterpret_cast<uint4 *>(sGH + o) = __ldg(reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(rs.gco) + o));
+        *reinterpret_cast<uint4 *>(sGH + 128 * Ns + o) =
+            __ldg(reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(rs.hco) + o));
+    }
+    const int64_t i = (int64_t)blockIdx.x * RT_B + tid;
+    const int64_t ic = i < n ? i : n - 1;  // threads past the end recompute the last point and store nothing
+    crf::tm_fence_before_sync();
+    __syncthreads();  // the tables have landed, the tensor-memory columns are allocated
+    crf::tm_fence_after_sync();
+    const unsigned tmq = crf::tm_quadrant(sTmBase, warp);
+    constexpr int NSTATE = (MODE == 1 || MODE == 2) ? 2 : 1;
+    const double zero[1] = {0.0};
+
+#pragma unroll 1
+    for (int st = 0; st < NSTATE; ++st) {
+        const unsigned tom = tmq + 4u * (Ns + 1) + 2u * (Ns + 1) * st;  // omega of this state
+        // the state: mode 1 = the second set of arrays, mode 2 = perturbed in place (multiply, then add: one rounding each)
+        auto in = [&](const double *a, const double *b, double sg, int64_t idx) {
+            if (st == 0 || MODE == 0 || MODE == 3) return a[idx];
+            return MODE == 1 ? b[idx] : __dadd_rn(a[idx], __dmul_rn(sg, b[idx]));
+        };
+        Ctx<1> c;
+        c.T[0] = in(io.T, io.T2, io.sigma, ic);
+        const double pi = in(io.p, io.p2, io.sigma_p, ic), Tu = c.T[0];
+        c.L[0] = log(Tu);
+        c.rT[0] = 1.0 / Tu;
+        const double lc02 = crf::kLog2e * (log(m.p_ref / CRF_R_GAS) - c.L[0]);
+        c.Csum[0] = pi * c.rT[0] * (1.0 / CRF_R_GAS);
+        const double oml = 1.0 - c.L[0];
+
+        double invW = 0.0;
+        for (int k0 = 0; k0 < Ns; k0 += 4) {
+            double y4[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {  // four row loads in flight
+                const int64_t idx = (int64_t)min(k0 + j, Ns - 1) * n + ic;
+                y4[j] = in(io.Y, io.Y2, io.sigma, idx);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k = k0 + j;
+                if (k >= Ns) break;
+                const double2 *g = reinterpret_cast<const double2 *>(sGH) + 8 * k;
+                const double2 *gs = g + (Tu <= g[3].y ? 0 : 4);
+                const double2 c01 = gs[0], c23 = gs[1], c45 = gs[2];
+                double g2 = fma(Tu, c45.x, c23.y);
+                g2 = fma(Tu, g2, c23.x);
+                g2 = fma(Tu, g2, c01.y);
+                g2 = fma(Tu, g2, gs[3].x);
+                g2 = fma(c45.y, c.rT[0], g2);
+                g2 = fma(c01.x, oml, g2);
+                const double z = y4[j] * g[7].y;
+                invW += z;
+                const double zd[2] = {z, exp2c(lc02 - g2)};
+                crf::tm_st<2>(tmq + 4u * k, zd);
+                crf::tm_st<1>(tom + 2u * k, zero);
+            }
+        }
+        const double one[2] = {1.0, 1.0};
+        crf::tm_st<2>(tmq + 4u * Ns, one);
+        crf::tm_st<1>(tom + 2u * Ns, zero);
+        crf::tm_wait_st();
+        const double rho = pi / (CRF_R_GAS * Tu * invW);
+        for (int k = 0; k < Ns; ++k) {  // C_k = rho Z_k
+            crf::TmRow<1> r;
+            crf::tm_ld<1>(tmq + 4u * k, r);
+            crf::tm_wait1<1>(r);
+            const double v[1] = {crf::tm_one(r) * rho};
+            crf::tm_st<1>(tmq + 4u * k, v);
+        }
+        crf::tm_wait_st();
+        if (MODE == 3 && i < n) {  // by-products of crf_rhs_pointwise (Eq. 1d)
+            if (io.rho) io.rho[i] = rho;
+            if (io.Wbar) io.Wbar[i] = 1.0 / invW;
+        }
+
+        for (int ci = 0; ci < rs.n_chunks; ++ci) {
+            const int4 ch = __ldg(rs.chunk + ci);
+            const char *blk = sTab + ch.z;
+            const int count = ch.y, o_troe = 48 * count + 32;  // one slot row (W = 1, maxown = 4) follows the records
+            switch (ch.x) {
+            case 0: thread_chunk_tm<0, false>(blk, count, o_troe, tmq, tom, c); break;
+            case 1: thread_chunk_tm<1, false>(blk, count, o_troe, tmq, tom, c); break;
+            case 2: thread_chunk_tm<2, false>(blk, count, o_troe, tmq, tom, c); break;
+            default: thread_chunk_tm<0, true>(blk, count, o_troe, tmq, tom, c); break;
+            }
+        }
+
+        // ---- omega of this state; a9: qdot = -sum_k h_k omega_k; mode 2, second state: the difference quotients
+        double qd = 0.0, cpm = 0.0, hm = 0.0;
+        for (int k = 0; k < Ns; ++k) {
+            const double2 *h = reinterpret_cast<const double2 *>(sGH + 128 * Ns) + 8 * k;
+            const double2 *hs = h + (Tu <= h[3].y ? 0 : 4);
+            const double2 c01 = hs[0], c23 = hs[1], c45 = hs[2];
+            double hk = fma(Tu, c45.x, c23.y);
+            hk = fma(Tu, hk, c23.x);
+            hk = fma(Tu, hk, c01.y);
+            hk = fma(Tu, hk, c01.x);
+            hk = fma(c45.y, c.rT[0], hk);
+            crf::TmRow<1> r, r0;
+            crf::tm_ld<1>(tom + 2u * k, r);
+            if (MODE == 2 && st == 1) crf::tm_ld<1>(tom - 2u * (Ns + 1) + 2u * k, r0);
+            crf::tm_wait1<1>(r);
+            if (MODE == 2 && st == 1) crf::tm_wait1<1>(r0);
+            const double w = crf::tm_one(r);
+            qd = fma(-hk, w, qd);
+            if (i < n) {
+                const int64_t o = (int64_t)k * n + i;
+                if (st == 0) {
+                    if (MODE != 2 || io.omega) io.omega[o] = w;
+                } else if (MODE == 1) {
+                    io.omega2[o] = w;
+                } else {
+                    io.omega2[o] = __dmul_rn(__dsub_rn(w, crf::tm_one(r0)), io.inv_sigma);
+                }
+            }
+            if (MODE == 3 && (io.cp || io.h || io.cpk)) {
+                // c_pk/R from the h/(RT) set (a_i = (i + 1) c_i); the mixture sums take Z_k = C_k / rho from the Y row again
+                double v = fma(Tu, 5.0 * c45.x, 4.0 * c23.y);
+                v = fma(Tu, v, 3.0 * c23.x);
+                v = fma(Tu, v, 2.0 * c01.y);
+                v = fma(Tu, v, c01.x);
+                const double zk = io.Y[(int64_t)k * n + ic] * h[7].y;
+                cpm = fma(zk, v, cpm);
+                hm = fma(zk, hk, hm);
+                if (io.cpk && i < n) io.cpk[(int64_t)k * n + i] = v * CRF_R_GAS;
+            }
+        }
+        if (i < n) {
+            const double q = qd * (CRF_R_GAS * Tu);
+            if (st == 0) {
+                if (MODE != 2 || io.qdot) io.qdot[i] = q;
+                if (MODE == 3 && io.cp) io.cp[i] = cpm * CRF_R_GAS;
+                if (MODE == 3 && io.h) io.h[i] = hm * (CRF_R_GAS * Tu);
+            } else if (MODE == 1) {
+                io.qdot2[i] = q;
+            }
+        }
+        if (MODE == 2) {  // qdot of the base state is needed again for the quotient: keep it in the dummy omega column
+            if (st == 0) {
+                const double v[1] = {qd * (CRF_R_GAS * Tu)};
+                crf::tm_st<1>(tom + 2u * Ns, v);
+                crf::tm_wait_st();
+            } else {
+                crf::TmRow<1> r;  // (tensor-memory accesses are warp-wide: never under a per-thread condition)
+                crf::tm_ld<1>(tom - 2u * (Ns + 1) + 2u * Ns, r);
+                crf::tm_wait1<1>(r);
+                if (i < n) io.qdot2[i] = __dmul_rn(__dsub_rn(qd * (CRF_R_GAS * Tu), crf::tm_one(r)), io.inv_sigma);
+            }
+        }
+    }
+    __syncthreads();
+    if (warp == 0) crf::tm_dealloc(sTmBase, tm_cols);
+}
+
+// whether the tensor-memory thread kernel serves this mechanism (columns: pairs 4 (Ns + 1), omega 2 (Ns + 1) per state)
+cudaError_t launch_thread_tm(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
+{
+    const int nstate = io.mode == 1 || io.mode == 2 ? 2 : 1;
+    unsigned cols = 32;
+    while ((int)cols < (4 + 2 * nstate) * (m.Ns + 1)) cols *= 2;
+    if (cols > 512) return cudaErrorInvalidValue;
+    // tables in shared memory, padded so that no more blocks are resident on an SM than the 512 columns hold
+    const size_t tables = (size_t)m.rs.stage_bytes + 256 * (size_t)m.Ns;
+    const size_t smem = std::max(tables, (size_t)(227 * 1024) / (512 / cols) - 2048);
+    const bool emit = io.cp || io.h || io.cpk || io.rho || io.Wbar;
+    void (*kernel)(DevTables, RatesIO, int64_t, unsigned) = rates_thread_tm_kernel<0>;
+    if (io.mode == 0 && emit) kernel = rates_thread_tm_kernel<3>;
+    if (io.mode == 1) kernel = rates_thread_tm_kernel<1>;
+    if (io.mode == 2) kernel = rates_thread_tm_kernel<2>;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kernel<<<(unsigned)((n + RT_B - 1) / RT_B), RT_B, smem, st>>>(m, io, n, cols);
+    crf_count_launch();
+    return cudaGetLastError();
+}
+
 cudaError_t launch_thread(const DevTables &m, const double *T, const double *p, const double *Y, int64_t n, double *omega,
                           double *qdot, cudaStream_t st)
 {
@@ -273,5 +557,17 @@ cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double 
                               double *omega, double *qdot, cudaStream_t st)
 {
     if (m.rs.W != 1 || m.rs.PPL != 4) return cudaErrorInvalidValue;
+    if (m.rs.tmem) return launch_thread_tm(m, rates_io(T, p, Y, omega, qdot), n, st);
     return launch_thread(m, T, p, Y, n, omega, qdot, st);
+}
+
+// the pair / difference-quotient / by-product calls on a small mechanism: the tensor-memory thread kernel, if the plan has it
+bool rates_thread_tm_serves(const DevTables &m, const RatesIO &io)
+{
+    const int nstate = io.mode == 1 || io.mode == 2 ? 2 : 1;
+    return m.rs.W == 1 && m.rs.PPL == 4 && m.rs.tmem && (4 + 2 * nstate) * (m.Ns + 1) <= 512;
+}
+cudaError_t launch_rates_thread_io(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
+{
+    return launch_thread_tm(m, io, n, st);
 }

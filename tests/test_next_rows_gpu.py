@@ -92,6 +92,30 @@ def test_pair_matches_oracle_and_single_calls(binding, oracle_mod, name):
     assert torch.equal(o1, s1) and torch.equal(q1, sq1) and torch.equal(o2, s2) and torch.equal(q2, sq2)
 
 
+@pytest.mark.parametrize("name", ["C1", "C2"])
+def test_pair_on_the_thread_kernel(binding, oracle_mod, name):
+    """Small mechanisms (default plan: one thread per point, state in tensor memory): the thread evaluates the two states
+    one after the other in one launch; bit-identical to two single calls, ragged n."""
+    desc = wl.make_mechanism(name)
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    info = gm.plan_info()
+    assert info["rates_kernel"] == "thread" and info["rates_tmem_cols"] > 0, info
+    n = 1000 + 37
+    a, b = _two_states(name, n)
+    da, db = parity.to_dev(a), parity.to_dev(b)
+    o1, q1, o2, q2 = gm.production_rates_pair(da["T"], da["p"], da["Y"], db["T"], db["p"], db["Y"])
+    s1, sq1 = gm.production_rates(da["T"], da["p"], da["Y"])
+    s2, sq2 = gm.production_rates(db["T"], db["p"], db["Y"])
+    assert torch.equal(o1, s1) and torch.equal(q1, sq1) and torch.equal(o2, s2) and torch.equal(q2, sq2)
+    ref = om.production_rates_pair(a["T"], a["p"], a["Y"], b["T"], b["p"], b["Y"])
+    assert np.max(np.abs(o2.cpu().numpy() - ref["omega2"]) / (parity.RATE_TOL * ref["S_omega2"] + 1e-30)) <= 1.0
+    # the shared-memory version of the same kernel (rates_tmem = 1) meets the same tolerance
+    g2 = binding.Mechanism(desc, options=dict(rates_tmem=1))
+    assert g2.plan_info()["rates_tmem_cols"] == 0
+    s3, _ = g2.production_rates(da["T"], da["p"], da["Y"])
+    assert np.max(np.abs(s3.cpu().numpy() - ref["omega"]) / (parity.RATE_TOL * ref["S_omega"] + 1e-30)) <= 1.0
+
+
 def test_pair_without_a_shared_launch(binding, oracle_mod):
     """A plan that cannot hold two states per lane answers the pair call with two launches: same numbers."""
     desc = wl.make_mechanism("C3")
