@@ -342,8 +342,7 @@ __device__ __forceinline__ void thread_chunk_tm(const char *blk, int count, int 
 }
 
 // MODE (RatesIO.mode; 3 = mode 0 with the by-products of crf_rhs_pointwise): in modes 1 and 2 the thread evaluates the
-// two states of its grid point one after the other (the tables are staged once; omega of the first state stays in
-// tensor memory until the quotient is formed).
+// two states of its grid point one after the other (the tables are staged once, the tensor-memory columns are reused).
 template <int MODE>
 __global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, RatesIO io, int64_t n, unsigned tm_cols)
 {
@@ -372,7 +371,7 @@ __global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, Rate
 
 #pragma unroll 1
     for (int st = 0; st < NSTATE; ++st) {
-        const unsigned tom = tmq + 4u * (Ns + 1) + 2u * (Ns + 1) * st;  // omega of this state
+        const unsigned tom = tmq + 4u * (Ns + 1);  // omega of this state (the columns are reused by the second state)
         // the state: mode 1 = the second set of arrays, mode 2 = perturbed in place (multiply, then add: one rounding each)
         auto in = [&](const double *a, const double *b, double sg, int64_t idx) {
             if (st == 0 || MODE == 0 || MODE == 3) return a[idx];
@@ -456,22 +455,22 @@ __global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, Rate
             hk = fma(Tu, hk, c01.y);
             hk = fma(Tu, hk, c01.x);
             hk = fma(c45.y, c.rT[0], hk);
-            crf::TmRow<1> r, r0;
+            crf::TmRow<1> r;
             crf::tm_ld<1>(tom + 2u * k, r);
-            if (MODE == 2 && st == 1) crf::tm_ld<1>(tom - 2u * (Ns + 1) + 2u * k, r0);
             crf::tm_wait1<1>(r);
-            if (MODE == 2 && st == 1) crf::tm_wait1<1>(r0);
             const double w = crf::tm_one(r);
             qd = fma(-hk, w, qd);
             if (i < n) {
                 const int64_t o = (int64_t)k * n + i;
-                if (st == 0) {
-                    if (MODE != 2 || io.omega) io.omega[o] = w;
-                } else if (MODE == 1) {
+                // (mode 2: omega of the base state waits in global memory, in `omega` if the caller wants it, else in the
+                // quotient's own row, and is read back by the same thread when the second state is done)
+                double *base = MODE == 2 && !io.omega ? io.omega2 : io.omega;
+                if (st == 0)
+                    base[o] = w;
+                else if (MODE == 1)
                     io.omega2[o] = w;
-                } else {
-                    io.omega2[o] = __dmul_rn(__dsub_rn(w, crf::tm_one(r0)), io.inv_sigma);
-                }
+                else
+                    io.omega2[o] = __dmul_rn(__dsub_rn(w, base[o]), io.inv_sigma);
             }
             if (MODE == 3 && (io.cp || io.h || io.cpk)) {
                 // c_pk/R from the h/(RT) set (a_i = (i + 1) c_i); the mixture sums take Z_k = C_k / rho from the Y row again
@@ -487,24 +486,15 @@ __global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, Rate
         }
         if (i < n) {
             const double q = qd * (CRF_R_GAS * Tu);
+            double *base = MODE == 2 && !io.qdot ? io.qdot2 : io.qdot;
             if (st == 0) {
-                if (MODE != 2 || io.qdot) io.qdot[i] = q;
+                base[i] = q;
                 if (MODE == 3 && io.cp) io.cp[i] = cpm * CRF_R_GAS;
                 if (MODE == 3 && io.h) io.h[i] = hm * (CRF_R_GAS * Tu);
             } else if (MODE == 1) {
                 io.qdot2[i] = q;
-            }
-        }
-        if (MODE == 2) {  // qdot of the base state is needed again for the quotient: keep it in the dummy omega column
-            if (st == 0) {
-                const double v[1] = {qd * (CRF_R_GAS * Tu)};
-                crf::tm_st<1>(tom + 2u * Ns, v);
-                crf::tm_wait_st();
             } else {
-                crf::TmRow<1> r;  // (tensor-memory accesses are warp-wide: never under a per-thread condition)
-                crf::tm_ld<1>(tom - 2u * (Ns + 1) + 2u * Ns, r);
-                crf::tm_wait1<1>(r);
-                if (i < n) io.qdot2[i] = __dmul_rn(__dsub_rn(qd * (CRF_R_GAS * Tu), crf::tm_one(r)), io.inv_sigma);
+                io.qdot2[i] = __dmul_rn(__dsub_rn(q, base[i]), io.inv_sigma);
             }
         }
     }
@@ -512,12 +502,11 @@ __global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, Rate
     if (warp == 0) crf::tm_dealloc(sTmBase, tm_cols);
 }
 
-// whether the tensor-memory thread kernel serves this mechanism (columns: pairs 4 (Ns + 1), omega 2 (Ns + 1) per state)
+// columns: the (C, d) pairs 4 (Ns + 1), omega 2 (Ns + 1)
 cudaError_t launch_thread_tm(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
 {
-    const int nstate = io.mode == 1 || io.mode == 2 ? 2 : 1;
     unsigned cols = 32;
-    while ((int)cols < (4 + 2 * nstate) * (m.Ns + 1)) cols *= 2;
+    while ((int)cols < 6 * (m.Ns + 1)) cols *= 2;
     if (cols > 512) return cudaErrorInvalidValue;
     // tables in shared memory, padded so that no more blocks are resident on an SM than the 512 columns hold
     const size_t tables = (size_t)m.rs.stage_bytes + 256 * (size_t)m.Ns;
@@ -564,8 +553,8 @@ cudaError_t launch_rates_smem(const DevTables &m, const double *T, const double 
 // the pair / difference-quotient / by-product calls on a small mechanism: the tensor-memory thread kernel, if the plan has it
 bool rates_thread_tm_serves(const DevTables &m, const RatesIO &io)
 {
-    const int nstate = io.mode == 1 || io.mode == 2 ? 2 : 1;
-    return m.rs.W == 1 && m.rs.PPL == 4 && m.rs.tmem && (4 + 2 * nstate) * (m.Ns + 1) <= 512;
+    (void)io;
+    return m.rs.W == 1 && m.rs.PPL == 4 && m.rs.tmem && 6 * (m.Ns + 1) <= 512;
 }
 cudaError_t launch_rates_thread_io(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
 {
