@@ -195,7 +195,10 @@ int crf_sem_diffusion(const crf_mech *mech, const double *h3, const double *T, c
  * crf_thermo, crf_production_rates and crf_mix_transport on each chunk and copies the seven
  * outputs back, chunks pipelined over internal streams.  All pointers are host pointers with
  * the layouts above (species-major with leading dimension n); pinned memory gives full copy
- * bandwidth.  Synchronous: returns when every output is in host memory. */
+ * bandwidth.  Synchronous: returns when every output is in host memory.  The outputs of one call form a group,
+ * (cp, h), (omega, qdot), (mu, lambda, rhoD): a group whose pointers are all NULL is neither computed nor copied (a
+ * Jacobian-vector product needs omega and qdot only: a third of the device-to-host traffic); a partly given group or
+ * no group at all is CRF_EINVAL. */
 int crf_step_host(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
                   double *cp, double *h, double *omega, double *qdot, double *mu, double *lambda, double *rhoD);
 

@@ -246,9 +246,10 @@ class Mechanism:
             mk = lambda *s: torch.empty(s, dtype=torch.float64)  # noqa: E731
             out = dict(cp=mk(n), h=mk(n), omega=mk(self.Ns, n), qdot=mk(n), mu=mk(n), lam=mk(n),
                        rhoD=mk(self.Ns, n))
+        def hp(key, shape):  # (an output left out of ``out``, or None, is not computed: crf.h)
+            return None if out.get(key) is None else _host(out[key], shape)
         _check(lib().crf_step_host(
             self._h, _host(T, (n,)), _host(p, (n,)), _host(Y, (self.Ns, n)), n,
-            _host(out["cp"], (n,)), _host(out["h"], (n,)), _host(out["omega"], (self.Ns, n)),
-            _host(out["qdot"], (n,)), _host(out["mu"], (n,)), _host(out["lam"], (n,)),
-            _host(out["rhoD"], (self.Ns, n))))
+            hp("cp", (n,)), hp("h", (n,)), hp("omega", (self.Ns, n)), hp("qdot", (n,)), hp("mu", (n,)), hp("lam", (n,)),
+            hp("rhoD", (self.Ns, n))))
         return out

@@ -460,8 +460,12 @@ int crf_step_host(crf_mech *mech, const double *T, const double *p, const double
                   double *omega, double *qdot, double *mu, double *lambda, double *rhoD)
 {
     CRF_CHECK_COMMON("crf_step_host")
-    if (!T || !p || !Y || !cp || !h || !omega || !qdot || !mu || !lambda || !rhoD)
-        return fail(CRF_EINVAL, "crf_step_host: null pointer");
+    if (!T || !p || !Y) return fail(CRF_EINVAL, "crf_step_host: null input pointer");
+    // outputs are wanted per call: (cp, h), (omega, qdot), (mu, lambda, rhoD); a group that is NULL is neither computed nor copied
+    const bool want_th = cp || h, want_ra = omega || qdot, want_tr = mu || lambda || rhoD;
+    if ((want_th && (!cp || !h)) || (want_ra && (!omega || !qdot)) || (want_tr && (!mu || !lambda || !rhoD)))
+        return fail(CRF_EINVAL, "crf_step_host: the outputs of a call must be given together or all be NULL");
+    if (!want_th && !want_ra && !want_tr) return fail(CRF_EINVAL, "crf_step_host: no output requested");
     const int Ns = mech->dev.Ns;
     const int64_t chunk = kChunk;
     const size_t rows = 7 + 3 * (size_t)Ns;
@@ -497,16 +501,22 @@ int crf_step_host(crf_mech *mech, const double *T, const double *p, const double
         CRF_TRY(cudaMemcpyAsync(dp, p + off, w, cudaMemcpyHostToDevice, st))
         CRF_TRY(cudaMemcpy2DAsync(dY, w, Y + off, (size_t)n * sizeof(double), w, Ns, cudaMemcpyHostToDevice, st))
         // kernels see a compact chunk: leading dimension c
-        CRF_TRY(launch_thermo(mech->dev, dT, dY, c, dcp, dh, st))
-        CRF_TRY(launch_rates(mech->dev, dT, dp, dY, c, dom, dq, st))
-        CRF_TRY(launch_transport(mech->dev, dT, dp, dY, c, dmu, dlam, drD, st))
-        CRF_TRY(cudaMemcpyAsync(cp + off, dcp, w, cudaMemcpyDeviceToHost, st))
-        CRF_TRY(cudaMemcpyAsync(h + off, dh, w, cudaMemcpyDeviceToHost, st))
-        CRF_TRY(cudaMemcpyAsync(qdot + off, dq, w, cudaMemcpyDeviceToHost, st))
-        CRF_TRY(cudaMemcpyAsync(mu + off, dmu, w, cudaMemcpyDeviceToHost, st))
-        CRF_TRY(cudaMemcpyAsync(lambda + off, dlam, w, cudaMemcpyDeviceToHost, st))
-        CRF_TRY(cudaMemcpy2DAsync(omega + off, (size_t)n * sizeof(double), dom, w, w, Ns, cudaMemcpyDeviceToHost, st))
-        CRF_TRY(cudaMemcpy2DAsync(rhoD + off, (size_t)n * sizeof(double), drD, w, w, Ns, cudaMemcpyDeviceToHost, st))
+        if (want_th) {
+            CRF_TRY(launch_thermo(mech->dev, dT, dY, c, dcp, dh, st))
+            CRF_TRY(cudaMemcpyAsync(cp + off, dcp, w, cudaMemcpyDeviceToHost, st))
+            CRF_TRY(cudaMemcpyAsync(h + off, dh, w, cudaMemcpyDeviceToHost, st))
+        }
+        if (want_ra) {
+            CRF_TRY(launch_rates(mech->dev, dT, dp, dY, c, dom, dq, st))
+            CRF_TRY(cudaMemcpyAsync(qdot + off, dq, w, cudaMemcpyDeviceToHost, st))
+            CRF_TRY(cudaMemcpy2DAsync(omega + off, (size_t)n * sizeof(double), dom, w, w, Ns, cudaMemcpyDeviceToHost, st))
+        }
+        if (want_tr) {
+            CRF_TRY(launch_transport(mech->dev, dT, dp, dY, c, dmu, dlam, drD, st))
+            CRF_TRY(cudaMemcpyAsync(mu + off, dmu, w, cudaMemcpyDeviceToHost, st))
+            CRF_TRY(cudaMemcpyAsync(lambda + off, dlam, w, cudaMemcpyDeviceToHost, st))
+            CRF_TRY(cudaMemcpy2DAsync(rhoD + off, (size_t)n * sizeof(double), drD, w, w, Ns, cudaMemcpyDeviceToHost, st))
+        }
     }
     for (int s = 0; s < kSlots; ++s) CRF_TRY(cudaStreamSynchronize(mech->pipe_stream[s]))
 #undef CRF_TRY

@@ -199,6 +199,22 @@ def test_step_host_matches_device_calls(binding, oracle_mod):
     parity.assert_parity(hsub, parity.run_oracle(om, sub), "step_host")
 
 
+def test_step_host_output_groups(binding, oracle_mod):
+    """crf_step_host computes and copies only the groups of outputs that are asked for."""
+    desc, gm, om = _mech_pair(binding, oracle_mod, "C3")
+    n = 70000  # more than one pipeline chunk
+    st = wl.make_state("C3", n=n, total=n)
+    host = {k: torch.from_numpy(v) for k, v in st.items()}
+    full = gm.step_host(host["T"], host["p"], host["Y"])
+    part = dict(omega=torch.empty(gm.Ns, n, dtype=torch.float64), qdot=torch.empty(n, dtype=torch.float64))
+    gm.step_host(host["T"], host["p"], host["Y"], part)
+    assert torch.equal(part["omega"], full["omega"]) and torch.equal(part["qdot"], full["qdot"])
+    with pytest.raises(binding.CrfError, match="together"):
+        gm.step_host(host["T"], host["p"], host["Y"], dict(omega=part["omega"]))
+    with pytest.raises(binding.CrfError, match="no output"):
+        gm.step_host(host["T"], host["p"], host["Y"], {})
+
+
 def test_fp64_probe(binding):
     r = binding.fp64_probe(2048)
     assert 1e12 < r < 4e13, r  # B200: 148 SM x 64 lanes x ~1.9 GHz = 1.8e13 FP64 instr/s nominal
