@@ -200,7 +200,7 @@ __device__ __forceinline__ void element(const DevTables &m, double *sm, const do
     // Jobs 0 .. Ns - 1: pass 1; Ns .. 2 Ns - 1: pass 2; 2 Ns: the heat flux.  The two input fields of job + 1 are fetched with
     // cp.async into a stage while job computes (each thread fetches and reads back its own point pairs).
     auto fetch = [&](int job) {
-        const int s = job < Ns ? job : job - Ns;
+        const int s = job < Ns ? job : 2 * Ns - 1 - job;  // (pass 2 walks the species backwards: the last ones of pass 1 are still in L2)
         const double *a = job == 2 * Ns ? T : Y + (int64_t)s * n, *b = job == 2 * Ns ? lam : rhoD + (int64_t)s * n;
         double2 *dst = sStage + (size_t)(job & 1) * 512 + threadIdx.x;
 #pragma unroll
@@ -247,7 +247,8 @@ __device__ __forceinline__ void element(const DevTables &m, double *sm, const do
     const double wgx = cW[g] * cW[2 * t] * jac, wgy = cW[g] * cW[2 * t + 1] * jac;  // w_j w_i |J| of the two points
     for (int s = 0; s <= Ns; ++s) {
         const bool heat = s == Ns;
-        const double Ws = heat ? 1.0 : __ldg(m.W + s), rWs = heat ? 1.0 : __ldg(m.rW + s);
+        const int sp = heat ? Ns : Ns - 1 - s;  // the species of this step
+        const double Ws = heat ? 1.0 : __ldg(m.W + sp), rWs = heat ? 1.0 : __ldg(m.rW + sp);
         if (!heat) {
             fetch(Ns + s + 1);
             cp_wait<1>();
@@ -289,7 +290,7 @@ __device__ __forceinline__ void element(const DevTables &m, double *sm, const do
         __syncthreads();
         double2 o[4];
         weak_div<WI>(sA, sB, sC, l, az, o);
-        double *dst = heat ? dT : dY + (int64_t)s * n;
+        double *dst = heat ? dT : dY + (int64_t)sp * n;
 #pragma unroll
         for (int q = 0; q < 4; ++q) *reinterpret_cast<double2 *>(dst + gbase + 64 * q) = o[q];
     }
