@@ -174,3 +174,53 @@ def test_new_calls_reject_bad_arguments(binding):
     outs[0] = None
     assert L.crf_rhs_pointwise(*args, *outs) == -1  # omega is required
     assert L.crf_rhs_pointwise(gm._h, st["T"].data_ptr(), st["p"].data_ptr(), st["Y"].data_ptr(), 0, *([None] * 10)) == 0
+
+
+@pytest.mark.parametrize("name", ["C2", "C5"])
+def test_next_rows_at_full_size_sampled(binding, oracle_mod, name):
+    """BASELINE.json's full sizes, in the launch configurations `bench.py --path rhs | jv | sem` times: sampled points
+    (the first and last, block boundaries, random ones) and sampled elements against the oracle, plus properties of the
+    whole fields."""
+    from oracle import sem_oracle
+    desc = wl.make_mechanism(name)
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    n = wl.config_points(name)
+    st = wl.make_state(name)
+    d = parity.to_dev(st)
+    rng = np.random.default_rng(321)
+    idx = np.unique(np.concatenate(([0, 1, 63, 64, 127, 128, n - 2, n - 1], rng.integers(0, n, 248))))
+    sub = dict(T=st["T"][idx], p=st["p"][idx], Y=np.ascontiguousarray(st["Y"][:, idx]))
+
+    def take(t):
+        return None if t is None else (t[:, idx] if t.dim() == 2 else t[idx]).cpu().numpy()
+
+    # crf_rhs_pointwise
+    rhs = gm.rhs_pointwise(d["T"], d["p"], d["Y"])
+    _check_rhs({k: take(v) for k, v in rhs.items()}, om.rhs_pointwise(**sub), f"rhs {name} full")
+    assert bool(torch.isfinite(rhs["rho"]).all()) and bool((rhs["rho"] > 0).all()) and bool((rhs["Wbar"] > 0).all())
+
+    # crf_production_rates_jv
+    v = {k: d[k] * (2 * torch.rand(d[k].shape, dtype=torch.float64, device="cuda", generator=torch.Generator("cuda").manual_seed(5)) - 1)
+         for k in ("T", "p", "Y")}
+    sigma = 1e-6
+    _, _, Jo, Jq = gm.production_rates_jv(d["T"], d["p"], d["Y"], v["T"], v["p"], v["Y"], sigma)
+    vs = {k: take(t) for k, t in v.items()}
+    ref = om.production_rates_jv(sub["T"], sub["p"], sub["Y"], vs["T"], vs["p"], vs["Y"], sigma)
+    assert np.max(np.abs(take(Jo) - ref["Jomega"]) / (parity.RATE_TOL * ref["S_Jomega"] + 1e-30 / sigma)) <= 1.0
+    assert np.max(np.abs(take(Jq) - ref["Jqdot"]) / (parity.RATE_TOL * ref["S_Jqdot"] + 1e-30 / sigma)) <= 1.0
+    assert bool(torch.isfinite(Jo).all())
+    del Jo, v
+
+    # crf_sem_diffusion on every element, sampled elements against the oracle (the operator is element-local)
+    nel = n // 512
+    h3 = np.random.default_rng(7).uniform(0.2e-3, 1.5e-3, (nel, 3))
+    dY, dT = gm.sem_diffusion(torch.from_numpy(h3).cuda(), d["T"], rhs["Wbar"], d["Y"], rhs["lam"], rhs["rhoD"])
+    els = np.unique(np.concatenate(([0, 1, nel - 1], rng.integers(0, nel, 5))))
+    pts = (els[:, None] * 512 + np.arange(512)[None, :]).reshape(-1)
+    pt = torch.from_numpy(pts).cuda()
+    args = (desc["W"], h3[els], st["T"][pts], rhs["Wbar"][pt].cpu().numpy(), np.ascontiguousarray(st["Y"][:, pts]),
+            rhs["lam"][pt].cpu().numpy(), rhs["rhoD"][:, pt].cpu().numpy())
+    sr, ss = sem_oracle.sem_diffusion(*args), sem_oracle.sem_diffusion_scale(*args)
+    assert np.max(np.abs(dY[:, pt].cpu().numpy() - sr["dY"]) / (1e-12 * ss["dY"] + 1e-300)) <= 1.0
+    assert np.max(np.abs(dT[pt].cpu().numpy() - sr["dT"]) / (1e-12 * ss["dT"] + 1e-300)) <= 1.0
+    assert bool(torch.isfinite(dY).all()) and bool(torch.isfinite(dT).all())
