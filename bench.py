@@ -440,6 +440,22 @@ def main():
                "ms_per_step": 1e3 * float(e2e_t.item()), "steps": Ke,
                "how": "crf_step_host: pinned host buffers, chunked H2D -> 3 kernels -> D2H over 3 streams, host wall clock"}
         del hout
+        # the mixed-precision variant (crf_step_host_f32: double arithmetic, outputs rounded to float on the device)
+        h32 = {k: torch.empty(sh, dtype=torch.float32).pin_memory() for k, sh in
+               dict(cp=(n,), h=(n,), omega=(Ns, n), qdot=(n,), mu=(n,), lam=(n,), rhoD=(Ns, n)).items()}
+        mech.step_host(host["T"], host["p"], host["Y"], h32)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            mech.step_host(host["T"], host["p"], host["Y"], h32)
+        torch.cuda.synchronize()
+        s32 = torch.tensor([(time.perf_counter() - t0) / Ke], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(s32, op=dist.ReduceOp.MAX)
+        e2e["f32_outputs"] = {"value": world * n / float(s32.item()), "unit": UNIT, "ms_per_step": 1e3 * float(s32.item()),
+                              "d2h_bytes_per_step": 4 * n * (2 * Ns + 5),
+                              "how": "crf_step_host_f32: the same path, outputs stored in single precision (half the D2H bytes)"}
+        del h32
 
     tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
     if world > 1:

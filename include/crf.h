@@ -202,6 +202,15 @@ int crf_sem_diffusion(const crf_mech *mech, const double *h3, const double *T, c
 int crf_step_host(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n,
                   double *cp, double *h, double *omega, double *qdot, double *mu, double *lambda, double *rhoD);
 
+/* Mixed-precision variant of crf_step_host: every step of the path is computed in double precision on the device, the
+ * OUTPUTS are rounded once (to nearest) to single precision on the device and returned as float arrays of the same
+ * layouts: half the device-to-host traffic of the end-to-end leg, which that traffic bounds.  This is the
+ * storage-in-reduced-precision technique the paper applies to its Krylov basis (FP32 basis, FP64 arithmetic,
+ * PAPER.md:59) and names as ongoing work, applied to what this library returns to a host-side
+ * consumer.  Each value is the float nearest to what crf_step_host returns.  Output groups as in crf_step_host. */
+int crf_step_host_f32(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, float *cp, float *h,
+                      float *omega, float *qdot, float *mu, float *lambda, float *rhoD);
+
 const char *crf_last_error(void);
 
 #ifdef __cplusplus

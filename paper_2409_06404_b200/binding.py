@@ -20,7 +20,7 @@ _lib = None
 EXPORTS = ("crf_mech_create", "crf_mech_destroy", "crf_mech_set_stream", "crf_mech_num_species",
            "crf_mech_num_reactions", "crf_thermo", "crf_thermo_species", "crf_production_rates",
            "crf_mix_transport", "crf_rhs_pointwise", "crf_production_rates_pair", "crf_production_rates_jv",
-           "crf_sem_diffusion", "crf_step_host", "crf_last_error")
+           "crf_sem_diffusion", "crf_step_host", "crf_step_host_f32", "crf_last_error")
 EXPORTS_DIAG = ("crf_mech_create_ex", "crf_mech_plan_info", "crf_fp64_probe", "crf_launch_count",
                 "crf_transport_schedule")
 
@@ -74,6 +74,7 @@ def lib() -> C.CDLL:
         L.crf_production_rates_jv.argtypes = [vp] + [dp] * 6 + [C.c_double, i64] + [dp] * 4
         L.crf_sem_diffusion.argtypes = [vp] + [dp] * 6 + [i64, dp, dp]
         L.crf_step_host.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
+        L.crf_step_host_f32.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
         L.crf_fp64_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.crf_launch_count.restype = C.c_int64
         L.crf_last_error.restype = C.c_char_p
@@ -246,9 +247,18 @@ class Mechanism:
             mk = lambda *s: torch.empty(s, dtype=torch.float64)  # noqa: E731
             out = dict(cp=mk(n), h=mk(n), omega=mk(self.Ns, n), qdot=mk(n), mu=mk(n), lam=mk(n),
                        rhoD=mk(self.Ns, n))
+        f32 = any(v is not None and v.dtype == torch.float32 for v in out.values())
+
         def hp(key, shape):  # (an output left out of ``out``, or None, is not computed: crf.h)
-            return None if out.get(key) is None else _host(out[key], shape)
-        _check(lib().crf_step_host(
+            if out.get(key) is None:
+                return None
+            t = out[key]
+            if f32:  # float32 outputs: crf_step_host_f32 (double arithmetic, outputs rounded once on the device)
+                if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+                    raise CrfError(f"expected a contiguous float32 host tensor of shape {tuple(shape)}")
+                return t.data_ptr()
+            return _host(t, shape)
+        _check((lib().crf_step_host_f32 if f32 else lib().crf_step_host)(
             self._h, _host(T, (n,)), _host(p, (n,)), _host(Y, (self.Ns, n)), n,
             hp("cp", (n,)), hp("h", (n,)), hp("omega", (self.Ns, n)), hp("qdot", (n,)), hp("mu", (n,)), hp("lam", (n,)),
             hp("rhoD", (self.Ns, n))))

@@ -455,33 +455,41 @@ int crf_sem_diffusion(const crf_mech *mech, const double *h3, const double *T, c
 }
 
 // Chunked host pipeline: slot s owns a stream and one device buffer holding, for a chunk of c points,
-// T, p, Y[Ns], cp, h, qdot, mu, lambda, omega[Ns], rhoD[Ns] (each row c doubles).
-int crf_step_host(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *cp, double *h,
-                  double *omega, double *qdot, double *mu, double *lambda, double *rhoD)
+// T, p, Y[Ns], cp, h, qdot, mu, lambda, omega[Ns], rhoD[Ns] (each row c doubles), then the same output rows as floats
+// (the single-precision staging of crf_step_host_f32).
+}  // extern "C"
+
+namespace {
+
+template <class Out>
+int step_host(const char *name, crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, Out *cp, Out *h,
+              Out *omega, Out *qdot, Out *mu, Out *lambda, Out *rhoD)
 {
-    CRF_CHECK_COMMON("crf_step_host")
-    if (!T || !p || !Y) return fail(CRF_EINVAL, "crf_step_host: null input pointer");
+    constexpr bool kF32 = sizeof(Out) == 4;
+    if (!mech) return fail(CRF_EINVAL, std::string(name) + ": null mechanism");
+    if (n < 0) return fail(CRF_EINVAL, std::string(name) + ": negative n");
+    if (n == 0) return CRF_OK;
+    if (!T || !p || !Y) return fail(CRF_EINVAL, std::string(name) + ": null input pointer");
     // outputs are wanted per call: (cp, h), (omega, qdot), (mu, lambda, rhoD); a group that is NULL is neither computed nor copied
     const bool want_th = cp || h, want_ra = omega || qdot, want_tr = mu || lambda || rhoD;
     if ((want_th && (!cp || !h)) || (want_ra && (!omega || !qdot)) || (want_tr && (!mu || !lambda || !rhoD)))
-        return fail(CRF_EINVAL, "crf_step_host: the outputs of a call must be given together or all be NULL");
-    if (!want_th && !want_ra && !want_tr) return fail(CRF_EINVAL, "crf_step_host: no output requested");
+        return fail(CRF_EINVAL, std::string(name) + ": the outputs of a call must be given together or all be NULL");
+    if (!want_th && !want_ra && !want_tr) return fail(CRF_EINVAL, std::string(name) + ": no output requested");
     const int Ns = mech->dev.Ns;
     const int64_t chunk = kChunk;
-    const size_t rows = 7 + 3 * (size_t)Ns;
+    const size_t rows = 7 + 3 * (size_t)Ns, out_rows = 5 + 2 * (size_t)Ns;
     cudaError_t e;
+#define CRF_TRY(call)                                              \
+    if ((e = (call)) != cudaSuccess) return fail_cuda(e, (std::string(name) + ": " #call).c_str());
     if (mech->pipe_chunk != chunk) {
         for (int s = 0; s < kSlots; ++s) {
-            if (!mech->pipe_stream[s]) {
-                e = cudaStreamCreateWithFlags(&mech->pipe_stream[s], cudaStreamNonBlocking);
-                if (e != cudaSuccess) return fail_cuda(e, "crf_step_host: stream");
-            }
+            if (!mech->pipe_stream[s]) CRF_TRY(cudaStreamCreateWithFlags(&mech->pipe_stream[s], cudaStreamNonBlocking))
             if (mech->pipe_buf[s]) cudaFree(mech->pipe_buf[s]);
             mech->pipe_buf[s] = nullptr;  // (a failed cudaMalloc below must not leave a dangling pointer for crf_mech_destroy)
-            e = cudaMalloc(&mech->pipe_buf[s], rows * chunk * sizeof(double));
+            e = cudaMalloc(&mech->pipe_buf[s], rows * chunk * sizeof(double) + out_rows * chunk * sizeof(float));
             if (e != cudaSuccess) {
                 mech->pipe_buf[s] = nullptr;
-                return fail_cuda(e, "crf_step_host: cudaMalloc");
+                return fail_cuda(e, (std::string(name) + ": cudaMalloc").c_str());
             }
         }
         mech->pipe_chunk = chunk;
@@ -494,33 +502,59 @@ int crf_step_host(crf_mech *mech, const double *T, const double *p, const double
         double *dT = b, *dp = b + chunk, *dY = b + 2 * chunk, *dcp = dY + (size_t)Ns * chunk, *dh = dcp + chunk,
                *dq = dh + chunk, *dmu = dq + chunk, *dlam = dmu + chunk, *dom = dlam + chunk,
                *drD = dom + (size_t)Ns * chunk;
+        float *f = reinterpret_cast<float *>(b + rows * chunk);  // the float image of the rows from dcp on, same order
         const size_t w = (size_t)c * sizeof(double);
-#define CRF_TRY(call)                                              \
-    if ((e = (call)) != cudaSuccess) return fail_cuda(e, "crf_step_host: " #call);
         CRF_TRY(cudaMemcpyAsync(dT, T + off, w, cudaMemcpyHostToDevice, st))
         CRF_TRY(cudaMemcpyAsync(dp, p + off, w, cudaMemcpyHostToDevice, st))
         CRF_TRY(cudaMemcpy2DAsync(dY, w, Y + off, (size_t)n * sizeof(double), w, Ns, cudaMemcpyHostToDevice, st))
+        // one output block of `nrow` rows (leading dimension c on the device, n on the host) back to the host, as doubles or,
+        // rounded once on the device, as floats
+        auto back = [&](Out *host, double *dev, int nrow) -> cudaError_t {
+            if (!kF32)
+                return cudaMemcpy2DAsync(host + off, (size_t)n * sizeof(Out), dev, w, w, nrow, cudaMemcpyDeviceToHost, st);
+            float *fs = f + (dev - dcp);  // (rows are c doubles apart on the device: the float image keeps the same indices)
+            cudaError_t ee = launch_f64_to_f32(dev, fs, (int64_t)nrow * c, st);
+            if (ee != cudaSuccess) return ee;
+            return cudaMemcpy2DAsync(host + off, (size_t)n * sizeof(Out), fs, (size_t)c * sizeof(float), (size_t)c * sizeof(float),
+                                     nrow, cudaMemcpyDeviceToHost, st);
+        };
         // kernels see a compact chunk: leading dimension c
         if (want_th) {
             CRF_TRY(launch_thermo(mech->dev, dT, dY, c, dcp, dh, st))
-            CRF_TRY(cudaMemcpyAsync(cp + off, dcp, w, cudaMemcpyDeviceToHost, st))
-            CRF_TRY(cudaMemcpyAsync(h + off, dh, w, cudaMemcpyDeviceToHost, st))
+            CRF_TRY(back(cp, dcp, 1))
+            CRF_TRY(back(h, dh, 1))
         }
         if (want_ra) {
             CRF_TRY(launch_rates(mech->dev, dT, dp, dY, c, dom, dq, st))
-            CRF_TRY(cudaMemcpyAsync(qdot + off, dq, w, cudaMemcpyDeviceToHost, st))
-            CRF_TRY(cudaMemcpy2DAsync(omega + off, (size_t)n * sizeof(double), dom, w, w, Ns, cudaMemcpyDeviceToHost, st))
+            CRF_TRY(back(qdot, dq, 1))
+            CRF_TRY(back(omega, dom, Ns))
         }
         if (want_tr) {
             CRF_TRY(launch_transport(mech->dev, dT, dp, dY, c, dmu, dlam, drD, st))
-            CRF_TRY(cudaMemcpyAsync(mu + off, dmu, w, cudaMemcpyDeviceToHost, st))
-            CRF_TRY(cudaMemcpyAsync(lambda + off, dlam, w, cudaMemcpyDeviceToHost, st))
-            CRF_TRY(cudaMemcpy2DAsync(rhoD + off, (size_t)n * sizeof(double), drD, w, w, Ns, cudaMemcpyDeviceToHost, st))
+            CRF_TRY(back(mu, dmu, 1))
+            CRF_TRY(back(lambda, dlam, 1))
+            CRF_TRY(back(rhoD, drD, Ns))
         }
     }
     for (int s = 0; s < kSlots; ++s) CRF_TRY(cudaStreamSynchronize(mech->pipe_stream[s]))
 #undef CRF_TRY
     return CRF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int crf_step_host(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *cp, double *h,
+                  double *omega, double *qdot, double *mu, double *lambda, double *rhoD)
+{
+    return step_host<double>("crf_step_host", mech, T, p, Y, n, cp, h, omega, qdot, mu, lambda, rhoD);
+}
+
+int crf_step_host_f32(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, float *cp, float *h,
+                      float *omega, float *qdot, float *mu, float *lambda, float *rhoD)
+{
+    return step_host<float>("crf_step_host_f32", mech, T, p, Y, n, cp, h, omega, qdot, mu, lambda, rhoD);
 }
 
 int crf_fp64_probe(int iters, double *inst_per_s)

@@ -50,6 +50,7 @@ cudaError_t launch_rates_thread_io(const DevTables &m, const RatesIO &io, int64_
 cudaError_t launch_sem_diffusion(const DevTables &m, const double *h3, const double *T, const double *Wbar, const double *Y,
                                  const double *lam, const double *rhoD, int64_t nel, double *dY, double *dT, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *inst_per_s);
+cudaError_t launch_f64_to_f32(const double *in, float *out, int64_t count, cudaStream_t st);
 // dynamic shared memory per block of the kernel the plan selects (0 for the generic kernels' own sizing): crf_plan_info
 size_t rates_dynamic_smem(const DevTables &m);
 size_t transport_dynamic_smem(const DevTables &m);

@@ -1,3 +1,4 @@
+#include <algorithm>
 // probe.cu -- sustained FP64 pipe rate: register-only DFMA chains on every SM.
 // 8 independent chains per thread, 256 threads per block, 8 blocks per SM: enough warps and ILP
 // to cover the DFMA latency, no memory traffic.  The measured instructions/s is the denominator
@@ -52,5 +53,22 @@ cudaError_t launch_fp64_probe(int iters, double *inst_per_s)
     if (e != cudaSuccess) return e;
     const double warp_inst = (double)blocks * 8.0 * (double)iters * 128.0;  // 8 warps x iters x 16 x 8 DFMA
     *inst_per_s = warp_inst * 32.0 / (ms * 1.0e-3);                        // thread-level FP64 instructions/s
+    return cudaGetLastError();
+}
+
+// ---- double -> float, round to nearest (the single-precision staging of crf_step_host_f32) ------------------------
+namespace {
+__global__ void __launch_bounds__(256) f64_to_f32_kernel(const double *__restrict__ in, float *__restrict__ out, int64_t count)
+{
+    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < count; i += (int64_t)gridDim.x * 256) out[i] = __double2float_rn(in[i]);
+}
+}  // namespace
+
+cudaError_t launch_f64_to_f32(const double *in, float *out, int64_t count, cudaStream_t st)
+{
+    if (count <= 0) return cudaSuccess;
+    const int64_t blocks = std::min<int64_t>((count + 255) / 256, 148 * 8);
+    f64_to_f32_kernel<<<(unsigned)blocks, 256, 0, st>>>(in, out, count);
+    crf_count_launch();
     return cudaGetLastError();
 }

@@ -215,6 +215,25 @@ def test_step_host_output_groups(binding, oracle_mod):
         gm.step_host(host["T"], host["p"], host["Y"], {})
 
 
+def test_step_host_f32_outputs(binding, oracle_mod):
+    """crf_step_host_f32: double arithmetic, outputs rounded once to float on the device: every value is the float
+    nearest to the double-precision result of crf_step_host (bit for bit), hence within 2^-24 of the oracle."""
+    desc, gm, om = _mech_pair(binding, oracle_mod, "C3")
+    n = 66000 + 3
+    st = wl.make_state("C3", n=n, total=n)
+    host = {k: torch.from_numpy(v) for k, v in st.items()}
+    full = gm.step_host(host["T"], host["p"], host["Y"])
+    out32 = {k: torch.empty(v.shape, dtype=torch.float32) for k, v in full.items()}
+    gm.step_host(host["T"], host["p"], host["Y"], out32)
+    for k, v in full.items():
+        assert torch.equal(out32[k], v.to(torch.float32)), k
+    ref = om.mix_transport(**{k: v[..., :512] for k, v in st.items()})
+    assert np.max(np.abs(out32["rhoD"][:, :512].numpy() - ref["rhoD"]) / ref["rhoD"]) <= 2.0 ** -24 * 1.001
+    part = dict(omega=torch.empty(gm.Ns, n, dtype=torch.float32), qdot=torch.empty(n, dtype=torch.float32))
+    gm.step_host(host["T"], host["p"], host["Y"], part)
+    assert torch.equal(part["omega"], out32["omega"])
+
+
 def test_fp64_probe(binding):
     r = binding.fp64_probe(2048)
     assert 1e12 < r < 4e13, r  # B200: 148 SM x 64 lanes x ~1.9 GHz = 1.8e13 FP64 instr/s nominal
