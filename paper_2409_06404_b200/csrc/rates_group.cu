@@ -34,6 +34,7 @@
 #include "crf_internal.h"
 #include "fastmath.cuh"
 #include "launch.h"
+#include "row_io.cuh"
 #include "tmem.cuh"
 
 namespace {
@@ -66,29 +67,8 @@ __device__ __forceinline__ uint4 ldsu4(const char *p) { return *reinterpret_cast
 __device__ __forceinline__ uint2 ldsu2(const char *p) { return *reinterpret_cast<const uint2 *>(p); }
 __device__ __forceinline__ double2 lds2(const char *p) { return *reinterpret_cast<const double2 *>(p); }
 
-// global rows: the PPL points of a lane are adjacent: i0, i0 + 1 (one 128-bit access per row when n is even)
-template <int PPL>
-__device__ __forceinline__ void load_row(const double *__restrict__ row, int64_t i0, int64_t n, bool vec, double (&v)[PPL])
-{
-    if (PPL == 2 && vec && i0 + 1 < n) {
-        const double2 t = *reinterpret_cast<const double2 *>(row + i0);
-        v[0] = t.x, v[PPL - 1] = t.y;
-    } else {
-#pragma unroll
-        for (int u = 0; u < PPL; ++u) v[u] = row[min(i0 + u, n - 1)];
-    }
-}
-template <int PPL>
-__device__ __forceinline__ void store_row(double *__restrict__ row, int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
-{
-    if (PPL == 2 && vec && i0 + 1 < n) {
-        *reinterpret_cast<double2 *>(row + i0) = make_double2(v[0], v[PPL - 1]);
-    } else {
-#pragma unroll
-        for (int u = 0; u < PPL; ++u)
-            if (i0 + u < n) row[i0 + u] = v[u];
-    }
-}
+using crf::load_row;
+using crf::store_row;
 
 // input row of the lane: MODE 0 the PPL adjacent points of `a`; MODE 1 (a[i], b[i]); MODE 2 (a[i], a[i] + sigma b[i]),
 // one rounding per operation so that the perturbed state is the one a host forms

@@ -24,6 +24,7 @@
 #include "crf_internal.h"
 #include "fastmath.cuh"
 #include "launch.h"
+#include "row_io.cuh"
 
 namespace {
 
@@ -122,29 +123,8 @@ __device__ __forceinline__ void stage_async(unsigned char *dst, const unsigned c
 }
 __device__ __forceinline__ void stage_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// the PPL points of a lane are adjacent: i0, i0 + 1 (one 128-bit access per row when n is even)
-template <int PPL>
-__device__ __forceinline__ void load_row(const double *__restrict__ row, int64_t i0, int64_t n, bool vec, double (&v)[PPL])
-{
-    if (PPL == 2 && vec && i0 + 1 < n) {
-        const double2 t = *reinterpret_cast<const double2 *>(row + i0);
-        v[0] = t.x, v[PPL - 1] = t.y;
-    } else {
-#pragma unroll
-        for (int u = 0; u < PPL; ++u) v[u] = row[min(i0 + u, n - 1)];
-    }
-}
-template <int PPL>
-__device__ __forceinline__ void store_row(double *__restrict__ row, int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
-{
-    if (PPL == 2 && vec && i0 + 1 < n) {
-        *reinterpret_cast<double2 *>(row + i0) = make_double2(v[0], v[PPL - 1]);
-    } else {
-#pragma unroll
-        for (int u = 0; u < PPL; ++u)
-            if (i0 + u < n) row[i0 + u] = v[u];
-    }
-}
+using crf::load_row;
+using crf::store_row;
 
 template <int W, int PPL>
 __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
