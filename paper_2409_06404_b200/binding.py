@@ -149,7 +149,11 @@ class Mechanism:
             lib().crf_mech_destroy(self._h)
             self._h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # interpreter shutdown: the module's globals (and the library handle) may be gone already
+            pass
 
     def _sync_stream(self):
         _check(lib().crf_mech_set_stream(self._h, C.c_void_p(torch.cuda.current_stream().cuda_stream)))
