@@ -211,6 +211,24 @@ int crf_step_host(crf_mech *mech, const double *T, const double *p, const double
 int crf_step_host_f32(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, float *cp, float *h,
                       float *omega, float *qdot, float *mu, float *lambda, float *rhoD);
 
+/* crf_step_host for callers that may not allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same path, host pointers, layouts and output groups as crf_step_host, but the device staging of the
+ * batch lives in a 16 MiB array that is part of the library's device image (every GPU that loads libcrf.so holds it
+ * until the process exits), and the work runs on the mechanism's stream (crf_mech_set_stream).  The call creates no
+ * stream and calls no cudaMalloc, cudaFree or other allocating routine; its only set-up is the address lookup of that
+ * array, once per device, on the first call there (with that device current, as for every call of a mechanism).
+ *   Limit: 7 ceil32(n) + 3 ceil32(Ns n) <= 2 097 152 doubles (ceil32: rounded up to a multiple of 32), i.e. about
+ *   2 097 152 / (7 + 3 Ns) points per call: 61 674 at Ns = 9, 5 808 at Ns = 118; crf_step_host_static_max_points
+ *   gives the exact number for a mechanism.  A larger n is CRF_EINVAL (crf_last_error names the limit); nothing runs.
+ * The array is shared by every call on the device, of any mechanism, and keeps the last call's contents (no part of it
+ * has to start at zero: a call writes every row before it reads it): calls that overlap on the GPU (other host threads
+ * or streams) race and must be serialised by the caller.  Synchronous: returns when the outputs are in host memory.
+ * Values are those of the device calls on a batch of n points (bit for bit those of crf_step_host for n <= 65 536). */
+int crf_step_host_static(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *cp, double *h,
+                         double *omega, double *qdot, double *mu, double *lambda, double *rhoD);
+/* the largest n crf_step_host_static accepts for this mechanism (negative: error code) */
+int64_t crf_step_host_static_max_points(const crf_mech *mech);
+
 const char *crf_last_error(void);
 
 #ifdef __cplusplus

@@ -20,7 +20,8 @@ _lib = None
 EXPORTS = ("crf_mech_create", "crf_mech_destroy", "crf_mech_set_stream", "crf_mech_num_species",
            "crf_mech_num_reactions", "crf_thermo", "crf_thermo_species", "crf_production_rates",
            "crf_mix_transport", "crf_rhs_pointwise", "crf_production_rates_pair", "crf_production_rates_jv",
-           "crf_sem_diffusion", "crf_step_host", "crf_step_host_f32", "crf_last_error")
+           "crf_sem_diffusion", "crf_step_host", "crf_step_host_f32", "crf_step_host_static",
+           "crf_step_host_static_max_points", "crf_last_error")
 EXPORTS_DIAG = ("crf_mech_create_ex", "crf_mech_plan_info", "crf_fp64_probe", "crf_launch_count",
                 "crf_transport_schedule")
 
@@ -75,6 +76,9 @@ def lib() -> C.CDLL:
         L.crf_sem_diffusion.argtypes = [vp] + [dp] * 6 + [i64, dp, dp]
         L.crf_step_host.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
         L.crf_step_host_f32.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
+        L.crf_step_host_static.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
+        L.crf_step_host_static_max_points.argtypes = [vp]
+        L.crf_step_host_static_max_points.restype = C.c_int64
         L.crf_fp64_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.crf_launch_count.restype = C.c_int64
         L.crf_last_error.restype = C.c_char_p
@@ -243,6 +247,27 @@ class Mechanism:
         _check(lib().crf_sem_diffusion(self._h, _dev(h3, (nel, 3)), _dev(T, (n,)), _dev(Wbar, (n,)), _dev(Y, (self.Ns, n)),
                                        _dev(lam, (n,)), _dev(rhoD, (self.Ns, n)), nel, _dev(dY, (self.Ns, n)), _dev(dT, (n,))))
         return dY, dT
+
+    def step_host_static_max_points(self) -> int:
+        """Largest batch ``step_host_static`` accepts for this mechanism (``crf_step_host_static_max_points``)."""
+        r = int(lib().crf_step_host_static_max_points(self._h))
+        if r < 0:
+            _check(r)
+        return r
+
+    def step_host_static(self, T, p, Y, out: dict) -> dict:
+        """``crf_step_host_static``: the whole path with HOST tensors and no allocation in the library: the device staging
+        is a 16 MiB array inside libcrf.so, so the batch is limited (``step_host_static_max_points``) and ``out`` (host
+        float64 tensors; groups as in ``step_host``) must be given.  Runs on torch's current stream; calls that overlap
+        on the GPU race on the shared array."""
+        n = T.numel()
+        self._sync_stream()
+        hp = lambda key, shape: None if out.get(key) is None else _host(out[key], shape)  # noqa: E731
+        _check(lib().crf_step_host_static(
+            self._h, _host(T, (n,)), _host(p, (n,)), _host(Y, (self.Ns, n)), n,
+            hp("cp", (n,)), hp("h", (n,)), hp("omega", (self.Ns, n)), hp("qdot", (n,)), hp("mu", (n,)), hp("lam", (n,)),
+            hp("rhoD", (self.Ns, n))))
+        return out
 
     def step_host(self, T, p, Y, out: dict | None = None) -> dict:
         """Whole path with HOST tensors (pinned for full bandwidth); returns host tensors."""

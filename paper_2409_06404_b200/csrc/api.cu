@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -562,6 +563,109 @@ int crf_fp64_probe(int iters, double *inst_per_s)
     if (iters < 1 || !inst_per_s) return fail(CRF_EINVAL, "crf_fp64_probe: bad argument");
     cudaError_t e = launch_fp64_probe(iters, inst_per_s);
     return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_fp64_probe");
+}
+
+}  // extern "C"
+
+// ---- crf_step_host_static: crf_step_host for callers that may not allocate ----------------------------------------
+// The device staging of the host-buffer call (inputs T, p, Y and the seven outputs of one batch) lives in a file-scope
+// device array instead of the cudaMalloc'ed pipeline buffers of crf_step_host: 16 MiB that every GPU which loads
+// libcrf.so holds until the process exits.  The call uses the mechanism's stream (crf_mech_set_stream), creates no
+// stream and calls no cudaMalloc / cudaFree; its only set-up is the address lookup of the array, once per device.
+// Every call on a device shares the array (also calls of different mechanisms): calls that overlap on the GPU race.
+// No part of the array has to start at zero (every row a call reads was written by the same call before), so nothing
+// is cleared; the array keeps the last call's contents.
+namespace {
+
+constexpr size_t kStaticDoubles = (size_t)2 << 20;  // 2 Mi doubles = 16 MiB
+static __device__ __align__(256) double g_static_scratch[kStaticDoubles];
+
+std::mutex g_static_mu;
+double *g_static_ptr[64] = {};  // the DEVICE address of g_static_scratch on each device (the name itself is a host-side stand-in)
+
+// blocks of the scratch start at multiples of 32 doubles (256 bytes)
+size_t pad32(size_t v) { return (v + 31) & ~(size_t)31; }
+size_t static_doubles(int Ns, int64_t n) { return 7 * pad32((size_t)n) + 3 * pad32((size_t)Ns * (size_t)n); }
+
+}  // namespace
+
+extern "C" {
+
+int64_t crf_step_host_static_max_points(const crf_mech *mech)
+{
+    if (!mech) return fail(CRF_EINVAL, "crf_step_host_static_max_points: null mechanism");
+    int64_t lo = 0, hi = (int64_t)kStaticDoubles;  // the largest n with static_doubles(Ns, n) <= kStaticDoubles
+    while (lo < hi) {
+        const int64_t mid = (lo + hi + 1) / 2;
+        if (static_doubles(mech->dev.Ns, mid) <= kStaticDoubles)
+            lo = mid;
+        else
+            hi = mid - 1;
+    }
+    return lo;
+}
+
+int crf_step_host_static(crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *cp, double *h,
+                         double *omega, double *qdot, double *mu, double *lambda, double *rhoD)
+{
+    const char *name = "crf_step_host_static";
+    if (!mech) return fail(CRF_EINVAL, std::string(name) + ": null mechanism");
+    if (n < 0) return fail(CRF_EINVAL, std::string(name) + ": negative n");
+    if (n == 0) return CRF_OK;
+    if (!T || !p || !Y) return fail(CRF_EINVAL, std::string(name) + ": null input pointer");
+    const bool want_th = cp || h, want_ra = omega || qdot, want_tr = mu || lambda || rhoD;
+    if ((want_th && (!cp || !h)) || (want_ra && (!omega || !qdot)) || (want_tr && (!mu || !lambda || !rhoD)))
+        return fail(CRF_EINVAL, std::string(name) + ": the outputs of a call must be given together or all be NULL");
+    if (!want_th && !want_ra && !want_tr) return fail(CRF_EINVAL, std::string(name) + ": no output requested");
+    const int Ns = mech->dev.Ns;
+    if (n > (int64_t)kStaticDoubles || static_doubles(Ns, n) > kStaticDoubles)
+        return fail(CRF_EINVAL, std::string(name) + ": n = " + std::to_string(n) + " points of " + std::to_string(Ns) +
+                                    " species exceed the 16 MiB static scratch (at most " +
+                                    std::to_string(crf_step_host_static_max_points(mech)) +
+                                    " points per call for this mechanism; use crf_step_host, which allocates)");
+    cudaError_t e;
+#define CRF_TRY(call)                                              \
+    if ((e = (call)) != cudaSuccess) return fail_cuda(e, (std::string(name) + ": " #call).c_str());
+    int dev = 0;
+    CRF_TRY(cudaGetDevice(&dev))
+    if (dev < 0 || dev >= 64) return fail(CRF_EINVAL, std::string(name) + ": device ordinal out of range");
+    double *b = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!g_static_ptr[dev]) {
+            void *q = nullptr;
+            CRF_TRY(cudaGetSymbolAddress(&q, g_static_scratch))
+            g_static_ptr[dev] = static_cast<double *>(q);
+        }
+        b = g_static_ptr[dev];
+    }
+    cudaStream_t st = mech->stream;
+    const size_t r1 = pad32((size_t)n), rN = pad32((size_t)Ns * (size_t)n);
+    double *dT = b, *dp = dT + r1, *dY = dp + r1, *dcp = dY + rN, *dh = dcp + r1, *dq = dh + r1, *dmu = dq + r1, *dlam = dmu + r1,
+           *dom = dlam + r1, *drD = dom + rN;
+    const size_t w = (size_t)n * sizeof(double);
+    CRF_TRY(cudaMemcpyAsync(dT, T, w, cudaMemcpyHostToDevice, st))
+    CRF_TRY(cudaMemcpyAsync(dp, p, w, cudaMemcpyHostToDevice, st))
+    CRF_TRY(cudaMemcpyAsync(dY, Y, w * Ns, cudaMemcpyHostToDevice, st))
+    if (want_th) {
+        CRF_TRY(launch_thermo(mech->dev, dT, dY, n, dcp, dh, st))
+        CRF_TRY(cudaMemcpyAsync(cp, dcp, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpyAsync(h, dh, w, cudaMemcpyDeviceToHost, st))
+    }
+    if (want_ra) {
+        CRF_TRY(launch_rates(mech->dev, dT, dp, dY, n, dom, dq, st))
+        CRF_TRY(cudaMemcpyAsync(qdot, dq, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpyAsync(omega, dom, w * Ns, cudaMemcpyDeviceToHost, st))
+    }
+    if (want_tr) {
+        CRF_TRY(launch_transport(mech->dev, dT, dp, dY, n, dmu, dlam, drD, st))
+        CRF_TRY(cudaMemcpyAsync(mu, dmu, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpyAsync(lambda, dlam, w, cudaMemcpyDeviceToHost, st))
+        CRF_TRY(cudaMemcpyAsync(rhoD, drD, w * Ns, cudaMemcpyDeviceToHost, st))
+    }
+    CRF_TRY(cudaStreamSynchronize(st))
+#undef CRF_TRY
+    return CRF_OK;
 }
 
 }  // extern "C"
