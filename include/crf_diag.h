@@ -42,7 +42,8 @@ typedef struct crf_plan_options {
     int32_t transport_PPL;    /* points per lane: 1 or 2 (TILED) */
     int32_t transport_panel;  /* column blocks per Wilke panel (TILED) */
     int32_t rates_tmem;       /* GROUP: 0 = u rows in tensor memory when they fit, 1 = in shared memory, 2 = require tensor memory */
-    int32_t reserved[7];      /* must be 0 */
+    int32_t transport_TS;     /* species per block of the pair tiles (TILED): 7 or 8; 0 = whichever the plan's estimate prefers */
+    int32_t reserved[6];      /* must be 0 */
 } crf_plan_options;
 
 /* What a mechanism will run. */
@@ -53,7 +54,8 @@ typedef struct crf_plan_info {
     int32_t transport_W, transport_PPL, transport_nb, transport_stage_blocks, transport_stage_bytes,
         transport_smem_bytes;
     int32_t rates_tmem_cols; /* tensor-memory columns a block of the GROUP kernel allocates (0: u rows in shared memory) */
-    int32_t reserved[7];
+    int32_t transport_TS;    /* species per block of the pair tiles (transport_nb counts these blocks) */
+    int32_t reserved[6];
 } crf_plan_info;
 
 /* crf_mech_create with an explicit plan request (options may be NULL = all automatic). */
@@ -69,7 +71,7 @@ int crf_fp64_probe(int iters, double *inst_per_s);
 int64_t crf_launch_count(void);
 
 /* Host-only (no device needed): the tile schedule crf_mech_create lays out for crf_mix_transport on a
- * mechanism whose species fill nb blocks of 8, dealt to W warps.  Writes up to `cap` tiles as
+ * mechanism whose species fill nb blocks (of 8 or 7 species), dealt to W warps.  Writes up to `cap` tiles as
  * int32 quadruples {round, kind (1 off-diagonal, 2 diagonal), jb, kb} to out and returns the number of tiles
  * of the schedule (which may exceed cap), or CRF_EINVAL. */
 int crf_transport_schedule(int nb, int W, int32_t *out, int cap);

@@ -190,7 +190,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
         info.rates_W = rpo.W, info.rates_PPL = 1, info.rates_Rc = rpo.Rc, info.rates_chunks = rpo.n_chunks;
     info.transport_kernel = tpo.W > 0 ? CRF_TRANSPORT_TILED : (tpo.small_n > 0 ? CRF_TRANSPORT_SMALL : CRF_TRANSPORT_GENERIC);
     if (tpo.W > 0)
-        info.transport_W = tpo.W, info.transport_PPL = tpo.PPL, info.transport_nb = tpo.nb,
+        info.transport_W = tpo.W, info.transport_PPL = tpo.PPL, info.transport_nb = tpo.nbp, info.transport_TS = tpo.TS,
         info.transport_stage_blocks = tpo.n_wilke + tpo.n_rounds, info.transport_stage_bytes = tpo.stage_bytes;
     if (opt.rates_kernel != CRF_RATES_AUTO && opt.rates_kernel != info.rates_kernel && Nr > 0)
         return fail(CRF_EUNSUPPORTED, "crf_mech_create_ex: the requested rates kernel does not admit this mechanism");
@@ -226,6 +226,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
     d.mu_c = D(omu), d.lam_c = D(olam), d.nDc = D(onD), d.wilke_c = D(owk), d.wq = D(owq);
     TransportPlan &tp = d.tp;
     tp.W = tpo.W, tp.PPL = tpo.PPL, tp.NsP = tpo.NsP, tp.nb = tpo.nb, tp.n_wilke = tpo.n_wilke, tp.n_rounds = tpo.n_rounds;
+    tp.TS = tpo.TS;
     tp.stage_bytes = tpo.stage_bytes;
     tp.small = D(tpo.small), tp.small_n = tpo.small_n;
     tp.rounds = reinterpret_cast<const int4 *>(base + tpo.rounds);
@@ -269,6 +270,8 @@ int crf_mech_create_ex(const crf_tables *t, const crf_plan_options *options, crf
     if (options) opt = *options;
     for (int32_t r : opt.reserved)
         if (r != 0) return fail(CRF_EINVAL, "crf_mech_create_ex: reserved option fields must be 0");
+    if (opt.transport_TS != 0 && opt.transport_TS != 7 && opt.transport_TS != 8)
+        return fail(CRF_EINVAL, "crf_mech_create_ex: transport_TS must be 0, 7 or 8");
     try {  // the host re-layout allocates: no C++ exception may cross the boundary
         return mech_create(t, opt, out);
     } catch (const std::bad_alloc &) {

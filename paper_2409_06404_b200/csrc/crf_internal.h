@@ -7,14 +7,15 @@
 #define CRF_R_GAS 8314.46261815324  // J/(kmol K)
 
 // Plan of the tiled crf_mix_transport kernel (transport_tiled.cu): species padded to blocks of 8, the pair
-// triangle cut into 8x8 tiles.  W warps share 32 PPL points; tiles are dealt to them in rounds whose tiles
+// triangle cut into 8x8 (or 7x7) tiles.  W warps share 32 PPL points; tiles are dealt to them in rounds whose tiles
 // touch disjoint species blocks (round-robin tournament over the blocks: a block's bye is its diagonal
 // tile), so the warps update disjoint rows of S.  A round's coefficients are one contiguous block that the
 // thread block copies global -> shared with cp.async while it works on the previous round.
 struct TransportPlan {
     int W;         // warps per block (1, 2, 4 or 8); 0 = no plan (generic kernel)
     int PPL;       // points per lane (1 or 2)
-    int NsP, nb;   // padded species count (multiple of 8) and number of 8-blocks
+    int NsP, nb;   // padded species count (rows of the state) and number of 8-blocks (Wilke phase)
+    int TS;        // tile edge of the pair phase: species blocks of 7 or 8
     int n_wilke;   // stage blocks of the Wilke phase (they come first in `rounds`)
     int n_rounds;  // stage blocks (rounds) of the pair phase
     int stage_bytes;          // largest stage block (multiple of 16)

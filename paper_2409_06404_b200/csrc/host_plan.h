@@ -24,6 +24,7 @@ struct BlockBuilder {
 // Offsets (into the block) of what a plan points to; resolved to device pointers after the upload.
 struct TransportPlanOffsets {
     int W = 0, PPL = 0, NsP = 0, nb = 0, n_wilke = 0, n_rounds = 0, stage_bytes = 0;
+    int TS = 8, nbp = 0;  // tile edge and species blocks of the pair phase
     int small_n = 0;
     size_t small = 0, rounds = 0, pair_coef = 0, wilke_cP = 0, sp = 0, Ddiag = 0;
 };

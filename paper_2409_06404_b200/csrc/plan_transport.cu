@@ -80,20 +80,49 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, const crf_plan_op
         return o;
     }
     if (want == CRF_TRANSPORT_SMALL) return o;  // unsupported request: Ns > 16
-    const int nb = (Ns + 7) / 8, NsP = 8 * nb;
-    // warps per point group: one per tile of a round-robin round (nb odd: (nb+1)/2, nb even: nb/2), at most 8;
-    // points per lane: 1 (16 warps per SM at 128 registers) or 2 (8 warps per SM, every coefficient load
-    // serves two points).  crf_plan_options.transport_W / transport_PPL override.
-    const int per_round = std::max(1, (nb + (nb & 1)) / 2);
-    int W = opt.transport_W;
-    if (W != 1 && W != 2 && W != 4 && W != 8) {
-        W = 1;
-        while (W < 8 && W < per_round) W *= 2;
-        if (nb <= 3) W = 1;  // a round of nb = 3 is one full tile and one diagonal tile: two warps would idle 28 %
-                             // (C3: W = 1 3.0 ms, W = 2 4.1 ms); the state is small, so the SM still holds 16 blocks
-    }
+    // warps per point group: one per tile of a round-robin round over the nbp pair blocks (nbp odd: (nbp+1)/2, nbp even:
+    // nbp/2), at most 8; points per lane: 1 (16 warps per SM at 128 registers) or 2 (8 warps per SM, every coefficient
+    // load serves two points).  crf_plan_options.transport_W / transport_PPL override.
+    auto warps_for = [&](int nbp) {
+        int W = opt.transport_W;
+        if (W != 1 && W != 2 && W != 4 && W != 8) {
+            const int per_round = std::max(1, (nbp + (nbp & 1)) / 2);
+            W = 1;
+            while (W < 8 && W < per_round) W *= 2;
+            if (nbp <= 3) W = 1;  // a round of nbp = 3 is one full tile and one diagonal tile: two warps would idle 28 %
+                                  // (C3: W = 1 3.0 ms, W = 2 4.1 ms); the state is small, so the SM still holds 16 blocks
+        }
+        return W;
+    };
+    // Tile edge of the pair phase: 8, or 7 where blocks of 7 species waste fewer padded pairs and idle warps (21 species:
+    // three 7-blocks hold exactly the 210 pairs, three 8-blocks evaluate 276; 53 species: eight 7-blocks make full rounds of
+    // four tiles, seven 8-blocks leave a warp with the half-size diagonal tile in every round).  The estimate is the
+    // warp-time of a point group: W (13 x the largest tile of every round + 3 x the Wilke terms of a warp).
+    auto cost_of = [&](int ts) {
+        const int nbp = (Ns + ts - 1) / ts, W = warps_for(nbp);
+        long pairs = 0;
+        for (auto &rd : schedule_rounds(nbp, W)) {
+            int worst = 0;
+            for (const Tile &tl : rd) worst = std::max(worst, tl.kind == 1 ? ts * ts : ts * (ts - 1) / 2);
+            pairs += worst;
+        }
+        const long wilke = (long)((nbp + W - 1) / W) * ts * ((ts * nbp + 3) / 4 * 4);
+        return W * (13 * pairs + 3 * wilke);
+    };
+    int TS = opt.transport_TS;
+    if (TS != 7 && TS != 8) TS = cost_of(7) < cost_of(8) ? 7 : 8;
+    // nb blocks of TS species (both phases); the state has NsP rows, all zero past Ns: the Wilke panels read their columns
+    // in groups of four and may run up to three rows past the last block
+    const int nb = (Ns + TS - 1) / TS, nbp = nb;
+    const int W = warps_for(nbp);
     const int PPL = opt.transport_PPL == 2 ? 2 : 1;
-    o.W = W, o.PPL = PPL, o.NsP = NsP, o.nb = nb;
+    // Wilke panels: up to kPanel column blocks (as many as keep a stage block within 20 KB: fewer, larger stage steps measured
+    // faster, C5 panel 3 -> 5 29.2 -> 28.8 ms, C4 15.5 -> 15.0 ms; crf_plan_options.transport_panel overrides)
+    const int kPanel = opt.transport_panel > 0 ? std::min(opt.transport_panel, nb) : std::max(1, std::min({nb, 5, 20480 / (W * 512)}));
+    int NsP = TS * nb;
+    for (int J0 = 0; J0 < nb; J0 += kPanel) NsP = std::max(NsP, TS * J0 + (TS * std::min(kPanel, nb - J0) + 3) / 4 * 4);
+    NsP += NsP & 1;
+    o.W = W, o.PPL = PPL, o.NsP = NsP, o.nb = nb, o.TS = TS, o.nbp = nbp;
 
     const int npair = Ns * (Ns + 1) / 2;
     auto pair_index = [&](int j, int k) {
@@ -118,33 +147,34 @@ TransportPlanOffsets build_transport_plan(const crf_tables *t, const crf_plan_op
         rdesc.push_back(make_int4((int)(8 * start), (int)(8 * (coef.size() - start)), flags, nJ));
         stage_bytes = std::max(stage_bytes, 8 * (coef.size() - start));
     };
-    // Wilke stage blocks: pass p covers the row blocks p W .. p W + W - 1 (one per warp), a panel covers up to
-    // kPanel column blocks (as many as keep the block within 20 KB: fewer, larger stage steps measured faster, C5 panel
-    // 3 -> 5 29.2 -> 28.8 ms, C4 15.5 -> 15.0 ms; crf_plan_options.transport_panel overrides); payload [W][8 rows][8 nJ columns] of c_kj (0 in padded rows/columns)
-    const int kPanel = opt.transport_panel > 0 ? std::min(opt.transport_panel, nb) : std::max(1, std::min({nb, 5, 20480 / (W * 512)})), npass = (nb + W - 1) / W;
+    // Wilke stage blocks: pass p covers the row blocks p W .. p W + W - 1 (one per warp), a panel covers up to kPanel column
+    // blocks; payload [W][TS rows][ld columns] of c_kj (0 in padded rows/columns), ld = TS nJ rounded up to a multiple of 4;
+    // descriptor w = nJ
+    const int npass = (nb + W - 1) / W;
     for (int ps = 0; ps < npass; ++ps)
         for (int J0 = 0; J0 < nb; J0 += kPanel) {
             const int nJ = std::min(kPanel, nb - J0);
             const size_t start = coef.size();
             coef.resize(start + hdr_d, 0.0);
+            const int ld = (TS * nJ + 3) / 4 * 4;
             for (int w = 0; w < W; ++w)
-                for (int a = 0; a < 8; ++a)
-                    for (int c = 0; c < 8 * nJ; ++c) {
-                        const int k = 8 * (ps * W + w) + a, j = 8 * J0 + c;
-                        coef.push_back(k < Ns && j < Ns ? 1.0 / std::sqrt(8.0 * (1.0 + t->W[k] / t->W[j])) : 0.0);
+                for (int a = 0; a < TS; ++a)
+                    for (int c = 0; c < ld; ++c) {
+                        const int k = TS * (ps * W + w) + a, j = TS * J0 + c;
+                        coef.push_back(c < TS * nJ && k < Ns && j < Ns ? 1.0 / std::sqrt(8.0 * (1.0 + t->W[k] / t->W[j])) : 0.0);
                     }
             close_block(start, J0 | ps << 8 | (J0 == 0) << 16 | (J0 + nJ == nb) << 17, nJ);
         }
     o.n_wilke = (int)rdesc.size();
-    for (auto &rd : schedule_rounds(nb, W)) {
+    for (auto &rd : schedule_rounds(nbp, W)) {
         const size_t start = coef.size();
         coef.resize(start + hdr_d, 0.0);
         for (int w = 0; w < (int)rd.size(); ++w) {
             const Tile &tl = rd[w];
             put_i(8 * start + 16 + 8 * (size_t)w, tl.kind | tl.jb << 8 | tl.kb << 16);
             put_i(8 * start + 16 + 8 * (size_t)w + 4, (int)(8 * (coef.size() - start)));
-            for (int a = 0; a < 8; ++a)
-                for (int c = tl.kind == 1 ? 0 : a + 1; c < 8; ++c) put_pair(coef, 8 * tl.jb + a, 8 * tl.kb + c);
+            for (int a = 0; a < TS; ++a)
+                for (int c = tl.kind == 1 ? 0 : a + 1; c < TS; ++c) put_pair(coef, TS * tl.jb + a, TS * tl.kb + c);
         }
         close_block(start, 0, 0);
     }

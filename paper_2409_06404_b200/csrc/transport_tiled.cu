@@ -43,26 +43,26 @@ __device__ __forceinline__ double cubic4(const double *__restrict__ c, double x)
 // state rows: [species][PPL][32] doubles; sZl / sSl point at this lane's column
 #define ROW(k, u) (((k) * PPL + (u)) * 32)
 
-// off-diagonal tile: species blocks jb < kb, 64 pairs; cf: the tile's coefficients in shared memory
-template <int PPL>
+// off-diagonal tile: species blocks jb < kb of TS species each, TS^2 pairs; cf: the tile's coefficients in shared memory
+template <int PPL, int TS>
 __device__ __forceinline__ void tile_offdiag(const double2 *cf, const double (&L)[PPL], const double *sZl, double *sSl,
                                              int jb, int kb, const double *tab)
 {
-    double zj[PPL][8], zk[PPL][8], sj[PPL][8], sk[PPL][8];
+    double zj[PPL][TS], zk[PPL][TS], sj[PPL][TS], sk[PPL][TS];
 #pragma unroll
     for (int u = 0; u < PPL; ++u)
 #pragma unroll
-        for (int a = 0; a < 8; ++a) {
-            zj[u][a] = sZl[ROW(8 * jb + a, u)];
-            zk[u][a] = sZl[ROW(8 * kb + a, u)];
+        for (int a = 0; a < TS; ++a) {
+            zj[u][a] = sZl[ROW(TS * jb + a, u)];
+            zk[u][a] = sZl[ROW(TS * kb + a, u)];
             sj[u][a] = 0.0;
             sk[u][a] = 0.0;
         }
 #pragma unroll
-    for (int a = 0; a < 8; ++a) {
+    for (int a = 0; a < TS; ++a) {
 #pragma unroll
-        for (int b = 0; b < 8; ++b) {
-            const double2 lo = cf[2 * (8 * a + b)], hi = cf[2 * (8 * a + b) + 1];
+        for (int b = 0; b < TS; ++b) {
+            const double2 lo = cf[2 * (TS * a + b)], hi = cf[2 * (TS * a + b) + 1];
 #pragma unroll
             for (int u = 0; u < PPL; ++u) {
                 const double e = exp2_tab64(fma(L[u], fma(L[u], fma(L[u], hi.y, hi.x), lo.y), lo.x), tab);
@@ -74,30 +74,30 @@ __device__ __forceinline__ void tile_offdiag(const double2 *cf, const double (&L
 #pragma unroll
     for (int u = 0; u < PPL; ++u)
 #pragma unroll
-        for (int a = 0; a < 8; ++a) {
-            sSl[ROW(8 * jb + a, u)] += sj[u][a];
-            sSl[ROW(8 * kb + a, u)] += sk[u][a];
+        for (int a = 0; a < TS; ++a) {
+            sSl[ROW(TS * jb + a, u)] += sj[u][a];
+            sSl[ROW(TS * kb + a, u)] += sk[u][a];
         }
 }
 
-// diagonal tile: pairs a < b inside block jb, 28 pairs
-template <int PPL>
+// diagonal tile: pairs a < b inside block jb, TS (TS - 1) / 2 pairs
+template <int PPL, int TS>
 __device__ __forceinline__ void tile_diag(const double2 *cf, const double (&L)[PPL], const double *sZl, double *sSl, int jb,
                                           const double *tab)
 {
-    double z[PPL][8], s[PPL][8];
+    double z[PPL][TS], s[PPL][TS];
 #pragma unroll
     for (int u = 0; u < PPL; ++u)
 #pragma unroll
-        for (int a = 0; a < 8; ++a) {
-            z[u][a] = sZl[ROW(8 * jb + a, u)];
+        for (int a = 0; a < TS; ++a) {
+            z[u][a] = sZl[ROW(TS * jb + a, u)];
             s[u][a] = 0.0;
         }
     int q = 0;
 #pragma unroll
-    for (int a = 0; a < 8; ++a) {
+    for (int a = 0; a < TS; ++a) {
 #pragma unroll
-        for (int b = a + 1; b < 8; ++b, ++q) {
+        for (int b = a + 1; b < TS; ++b, ++q) {
             const double2 lo = cf[2 * q], hi = cf[2 * q + 1];
 #pragma unroll
             for (int u = 0; u < PPL; ++u) {
@@ -110,7 +110,7 @@ __device__ __forceinline__ void tile_diag(const double2 *cf, const double (&L)[P
 #pragma unroll
     for (int u = 0; u < PPL; ++u)
 #pragma unroll
-        for (int a = 0; a < 8; ++a) sSl[ROW(8 * jb + a, u)] += s[u][a];
+        for (int a = 0; a < TS; ++a) sSl[ROW(TS * jb + a, u)] += s[u][a];
 }
 
 __device__ __forceinline__ void stage_async(unsigned char *dst, const unsigned char *src, int bytes, int tid, int nthreads)
@@ -126,7 +126,7 @@ __device__ __forceinline__ void stage_wait() { asm volatile("cp.async.wait_all;"
 using crf::load_row;
 using crf::store_row;
 
-template <int W, int PPL>
+template <int W, int PPL, int TS>
 __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
     transport_tiled_kernel(DevTables m, const double *__restrict__ T, const double *__restrict__ Y, int64_t n,
                            double *__restrict__ mu, double *__restrict__ lambda, double *__restrict__ rhoD)
@@ -208,7 +208,7 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
     for (int u = 0; u < PPL; ++u) mu_p[u] = 0.0;
     const int nwk = tp.n_wilke;
     {
-        double A[PPL][8], B[PPL][8], C[PPL][8];
+        double A[PPL][TS], B[PPL][TS], C[PPL][TS];
         for (int s = 0; s < nwk; ++s) {
             stage_wait();
             __syncthreads();  // block s has landed; everyone is done with block s - 1
@@ -222,25 +222,26 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
 #pragma unroll
                 for (int u = 0; u < PPL; ++u)
 #pragma unroll
-                    for (int a = 0; a < 8; ++a) A[u][a] = B[u][a] = C[u][a] = 0.0;
+                    for (int a = 0; a < TS; ++a) A[u][a] = B[u][a] = C[u][a] = 0.0;
             }
-            const int ld = 8 * nJ;  // row length of the slab
-            const double *cw = reinterpret_cast<const double *>(blk + HDR) + warp * 8 * ld;
+            // row length of the slab: the nJ column blocks, rounded up to whole groups of four columns (zero coefficients)
+            const int ld = TS == 8 ? 8 * nJ : (TS * nJ + 3) & ~3;
+            const double *cw = reinterpret_cast<const double *>(blk + HDR) + warp * TS * ld;
             // four columns at a time: 12 right-hand-side values in registers leave room for the compiler to
             // keep several coefficient loads in flight
-            for (int j4 = 0; j4 < 2 * nJ; ++j4) {
+            for (int j4 = 0; j4 < (TS == 8 ? 2 * nJ : ld >> 2); ++j4) {
 #pragma unroll
                 for (int u = 0; u < PPL; ++u) {
                     double u0[4], u1[4], u2[4];
 #pragma unroll
                     for (int b = 0; b < 4; ++b) {
-                        u0[b] = sZl[ROW(8 * J0 + 4 * j4 + b, u)];
-                        const double r = sSl[ROW(8 * J0 + 4 * j4 + b, u)];
+                        u0[b] = sZl[ROW(TS * J0 + 4 * j4 + b, u)];
+                        const double r = sSl[ROW(TS * J0 + 4 * j4 + b, u)];
                         u1[b] = u0[b] * r;
                         u2[b] = u1[b] * r;
                     }
 #pragma unroll
-                    for (int a = 0; a < 8; ++a) {
+                    for (int a = 0; a < TS; ++a) {
                         const double2 c01 = *reinterpret_cast<const double2 *>(cw + a * ld + 4 * j4);
                         const double2 c23 = *reinterpret_cast<const double2 *>(cw + a * ld + 4 * j4 + 2);
                         A[u][a] = fma(c01.x, u0[0], A[u][a]);
@@ -260,8 +261,8 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
             }
             if (ds.z & (1 << 17)) {
 #pragma unroll
-                for (int a = 0; a < 8; ++a) {
-                    const int k = 8 * I + a;
+                for (int a = 0; a < TS; ++a) {
+                    const int k = TS * I + a;
                     if (k < Ns) {
                         const double wk = __ldg(tp.sp + 12 * k + 9);
 #pragma unroll
@@ -322,9 +323,9 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
         const int kind = d.x & 0xff, jb = (d.x >> 8) & 0xff, kb = (d.x >> 16) & 0xff;
         const double2 *cf = reinterpret_cast<const double2 *>(blk + d.y);
         if (kind == 1)
-            tile_offdiag<PPL>(cf, L, sZl, sSl, jb, kb, sTab);
+            tile_offdiag<PPL, TS>(cf, L, sZl, sSl, jb, kb, sTab);
         else if (kind == 2)
-            tile_diag<PPL>(cf, L, sZl, sSl, jb, sTab);
+            tile_diag<PPL, TS>(cf, L, sZl, sSl, jb, sTab);
         stage_wait();
         __syncthreads();
     }
@@ -357,19 +358,26 @@ __global__ void __launch_bounds__(32 * W, 16 / (W * PPL))
     }
 }
 
+template <int W, int PPL, int TS>
+cudaError_t launch_w2(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu, double *lambda,
+                     double *rhoD, cudaStream_t st)
+{
+    const size_t smem = transport_tiled_dynamic_smem(m);
+    cudaError_t e = cudaFuncSetAttribute(transport_tiled_kernel<W, PPL, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem);
+    if (e != cudaSuccess) return e;
+    const int64_t per_block = 32 * PPL;
+    transport_tiled_kernel<W, PPL, TS><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, Y, n, mu,
+                                                                                                     lambda, rhoD);
+    crf_count_launch();
+    return cudaGetLastError();
+}
+
 template <int W, int PPL>
 cudaError_t launch_w(const DevTables &m, const double *T, const double *Y, int64_t n, double *mu, double *lambda,
                      double *rhoD, cudaStream_t st)
 {
-    const size_t smem = transport_tiled_dynamic_smem(m);
-    cudaError_t e = cudaFuncSetAttribute(transport_tiled_kernel<W, PPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)smem);
-    if (e != cudaSuccess) return e;
-    const int64_t per_block = 32 * PPL;
-    transport_tiled_kernel<W, PPL><<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, T, Y, n, mu,
-                                                                                                     lambda, rhoD);
-    crf_count_launch();
-    return cudaGetLastError();
+    return m.tp.TS == 7 ? launch_w2<W, PPL, 7>(m, T, Y, n, mu, lambda, rhoD, st) : launch_w2<W, PPL, 8>(m, T, Y, n, mu, lambda, rhoD, st);
 }
 
 }  // namespace

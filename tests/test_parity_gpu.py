@@ -244,6 +244,10 @@ PLAN_OVERRIDES = [
     dict(transport_kernel="tiled", transport_W=4),         # rounds split over fewer warps than tiles
     dict(transport_kernel="tiled", transport_W=1, transport_PPL=2),
     dict(transport_kernel="tiled", transport_panel=1),     # one column block per Wilke panel (most stage steps)
+    dict(transport_kernel="tiled", transport_TS=8),        # species blocks of 8 in both phases
+    dict(transport_kernel="tiled", transport_TS=7),        # blocks of 7 (the automatic choice for C3 and C4; C5: 17 blocks, split rounds)
+    dict(transport_kernel="tiled", transport_TS=7, transport_PPL=2),
+    dict(transport_kernel="tiled", transport_TS=7, transport_W=2, transport_panel=2),  # Wilke panels that end off a multiple of 4
     dict(rates_kernel="group", rates_W=8, rates_PPL=1),
     dict(rates_kernel="group", rates_W=4, rates_PPL=2, rates_Rc=32),   # many small chunks
     dict(rates_kernel="group", rates_W=16, rates_PPL=2),
