@@ -45,6 +45,9 @@ def parse():
                     help="three: crf_thermo + crf_production_rates + crf_mix_transport (the default step); rhs: one "
                          "crf_rhs_pointwise call (SURVEY 8(f)1); jv: one crf_production_rates_jv call (8(f)2); sem: one "
                          "crf_sem_diffusion call on the outputs of crf_rhs_pointwise (8(f)3)")
+    ap.add_argument("--plan", nargs="*", default=[], metavar="KEY=VALUE",
+                    help="explicit kernel plan (crf_plan_options of include/crf_diag.h, e.g. thermo_sets=2); default: the "
+                         "library's automatic plan.  Recorded in config.plan")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -357,7 +360,8 @@ def main():
     n = args.points or wl.config_points(name)
     offset, n, total = shard.weak_range(n, rank, world)
     desc = wl.make_mechanism(name)
-    mech = binding.Mechanism(desc)
+    plan = {k: (int(v) if v.lstrip("-").isdigit() else v) for k, v in (kv.split("=", 1) for kv in args.plan)}
+    mech = binding.Mechanism(desc, plan or None)
     Ns = mech.Ns
     st = wl.make_state(name, n=n, offset=offset, total=total)
     host = {k: torch.from_numpy(v).pin_memory() for k, v in st.items()}
@@ -520,7 +524,8 @@ def main():
 
     line = {"metric": METRIC, "value": world * n * K / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(name, n, world),
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(config_dict(name, n, world), plan=plan or "automatic", plan_info=mech.plan_info()),
             "clocks": clock_info, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
             "kernels": kernels}
     print(json.dumps(line))

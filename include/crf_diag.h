@@ -43,7 +43,12 @@ typedef struct crf_plan_options {
     int32_t transport_panel;  /* column blocks per Wilke panel (TILED) */
     int32_t rates_tmem;       /* GROUP: 0 = u rows in tensor memory when they fit, 1 = in shared memory, 2 = require tensor memory */
     int32_t transport_TS;     /* species per block of the pair tiles (TILED): 7 or 8; 0 = whichever the plan's estimate prefers */
-    int32_t reserved[6];      /* must be 0 */
+    int32_t thermo_sets;      /* crf_thermo: 2 = both NASA-7 sets of a species at warp-uniform addresses, the point's mass fraction
+                               * routed to the set of its range (twelve FMAs per species and point; the default: 0.80-0.86 of
+                               * the HBM roofline on every config); 1 = every lane reads the set of its own range (six FMAs;
+                               * faster, 0.91-0.93, where the points of a warp share their ranges, as in spatially coherent
+                               * fields, slower, 0.74, where they do not); 0 = default */
+    int32_t reserved[5];      /* must be 0 */
 } crf_plan_options;
 
 /* What a mechanism will run. */
@@ -55,7 +60,8 @@ typedef struct crf_plan_info {
         transport_smem_bytes;
     int32_t rates_tmem_cols; /* tensor-memory columns a block of the GROUP kernel allocates (0: u rows in shared memory) */
     int32_t transport_TS;    /* species per block of the pair tiles (transport_nb counts these blocks) */
-    int32_t reserved[6];
+    int32_t thermo_sets;     /* 1 or 2 (crf_plan_options.thermo_sets) */
+    int32_t reserved[5];
 } crf_plan_info;
 
 /* crf_mech_create with an explicit plan request (options may be NULL = all automatic). */

@@ -32,8 +32,9 @@ TRANSPORT_KERNELS = {"auto": 0, "generic": 1, "small": 2, "tiled": 3}
 class PlanOptions(C.Structure):
     """ctypes mirror of ``crf_plan_options`` (include/crf_diag.h)."""
     _fields_ = [(n, C.c_int32) for n in ("rates_kernel", "rates_W", "rates_PPL", "rates_Rc", "transport_kernel",
-                                         "transport_W", "transport_PPL", "transport_panel", "rates_tmem", "transport_TS")] \
-        + [("reserved", C.c_int32 * 6)]
+                                         "transport_W", "transport_PPL", "transport_panel", "rates_tmem", "transport_TS",
+                                         "thermo_sets")] \
+        + [("reserved", C.c_int32 * 5)]
 
 
 class PlanInfo(C.Structure):
@@ -41,8 +42,9 @@ class PlanInfo(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("rates_kernel", "rates_W", "rates_PPL", "rates_Rc", "rates_chunks",
                                          "rates_stage_bytes", "rates_smem_bytes", "transport_kernel", "transport_W",
                                          "transport_PPL", "transport_nb", "transport_stage_blocks",
-                                         "transport_stage_bytes", "transport_smem_bytes", "rates_tmem_cols", "transport_TS")] \
-        + [("reserved", C.c_int32 * 6)]
+                                         "transport_stage_bytes", "transport_smem_bytes", "rates_tmem_cols", "transport_TS",
+                                         "thermo_sets")] \
+        + [("reserved", C.c_int32 * 5)]
 
 
 class CrfError(RuntimeError):

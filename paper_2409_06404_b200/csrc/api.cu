@@ -192,6 +192,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
     if (tpo.W > 0)
         info.transport_W = tpo.W, info.transport_PPL = tpo.PPL, info.transport_nb = tpo.nbp, info.transport_TS = tpo.TS,
         info.transport_stage_blocks = tpo.n_wilke + tpo.n_rounds, info.transport_stage_bytes = tpo.stage_bytes;
+    info.thermo_sets = opt.thermo_sets == 1 ? 1 : 2;
     if (opt.rates_kernel != CRF_RATES_AUTO && opt.rates_kernel != info.rates_kernel && Nr > 0)
         return fail(CRF_EUNSUPPORTED, "crf_mech_create_ex: the requested rates kernel does not admit this mechanism");
     if (opt.transport_kernel != CRF_TRANSPORT_AUTO && opt.transport_kernel != info.transport_kernel)
@@ -223,6 +224,7 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
     d.lnA0 = D(olnA0), d.beta0 = D(ob0), d.Ea0_R = D(oE0), d.alpha = D(oal), d.rT3 = D(orT3), d.rT1 = D(orT1),
     d.T2 = D(oT2);
     d.thermo_tab = D(otht);
+    d.thermo_sets = opt.thermo_sets == 1 ? 1 : 2;
     d.mu_c = D(omu), d.lam_c = D(olam), d.nDc = D(onD), d.wilke_c = D(owk), d.wq = D(owq);
     TransportPlan &tp = d.tp;
     tp.W = tpo.W, tp.PPL = tpo.PPL, tp.NsP = tpo.NsP, tp.nb = tpo.nb, tp.n_wilke = tpo.n_wilke, tp.n_rounds = tpo.n_rounds;
@@ -272,6 +274,7 @@ int crf_mech_create_ex(const crf_tables *t, const crf_plan_options *options, crf
         if (r != 0) return fail(CRF_EINVAL, "crf_mech_create_ex: reserved option fields must be 0");
     if (opt.transport_TS != 0 && opt.transport_TS != 7 && opt.transport_TS != 8)
         return fail(CRF_EINVAL, "crf_mech_create_ex: transport_TS must be 0, 7 or 8");
+    if (opt.thermo_sets < 0 || opt.thermo_sets > 2) return fail(CRF_EINVAL, "crf_mech_create_ex: thermo_sets must be 0, 1 or 2");
     try {  // the host re-layout allocates: no C++ exception may cross the boundary
         return mech_create(t, opt, out);
     } catch (const std::bad_alloc &) {

@@ -136,6 +136,7 @@ struct DevTables {
     const double *cpc, *hc, *gc, *sc;  // sc[6]: s/R = c0 ln T + T(c1 + ...c4) + c5
     // crf_thermo (thermo.cu): [Ns][14] = {a1..a5, a6} / W_k of the low range, of the high range, then T_mid, pad
     const double *thermo_tab;
+    int thermo_sets;  // 1: a lane reads the coefficient set of its range; 2: both sets at uniform addresses (thermo.cu)
     // reactions (sorted elementary | third-body | falloff)
     const double *lnA, *beta, *Ea_R, *dnu;  // [Nr]; dnu = sum nu'' - sum nu'
     const int16_t *reac, *prod;             // [3][Nr]

@@ -11,6 +11,10 @@
 // per block into shared memory; a thread owns two adjacent points (128-bit loads of the Y rows), the species loop
 // is unrolled by four so that four row loads are in flight per thread, and a block walks several point groups.
 // The range select T <= T_mid compares the bit patterns as integers (both are positive): no FP64 pipe instruction.
+// Two instances (crf_plan_options.thermo_sets).  <false>: a lane reads the coefficient set of its own range: a broadcast (one
+// shared-memory wavefront per load) where the lanes of a warp agree, one wavefront per quarter warp where they do not (fields
+// without spatial coherence in T: the shared-memory pipe then takes as long as the HBM stream).  <true>, the default: both
+// sets at warp-uniform addresses and twelve FMAs, the mass fraction routed to the set of the point's range.
 #include "crf_internal.h"
 #include <algorithm>
 
@@ -39,6 +43,29 @@ __device__ __forceinline__ void thermo_species_step(const double *__restrict__ t
     }
 }
 
+// The same sums with BOTH coefficient sets read at warp-uniform addresses (six broadcast loads: one shared-memory wavefront
+// each) and the point's mass fraction routed to the set of its range: twelve FMAs per species and point instead of six,
+// a quarter of the shared-memory wavefronts when the lanes of a warp sit in different ranges (crf_plan_options.thermo_sets).
+template <int P>
+__device__ __forceinline__ void thermo_species_step_both(const double *__restrict__ tab, int k, const double (&y)[P],
+                                                         const long long (&Tbits)[P], double (&M)[6][P])
+{
+    const double2 *c = reinterpret_cast<const double2 *>(tab + TH_STRIDE * k);
+    const long long tmid = __double_as_longlong(tab[TH_STRIDE * k + 12]);
+    const double2 l01 = c[0], l23 = c[1], l45 = c[2], h01 = c[3], h23 = c[4], h45 = c[5];
+#pragma unroll
+    for (int u = 0; u < P; ++u) {
+        const bool lo = Tbits[u] <= tmid;
+        const double yl = lo ? y[u] : 0.0, yh = lo ? 0.0 : y[u];
+        M[0][u] = fma(yl, l01.x, M[0][u]), M[1][u] = fma(yl, l01.y, M[1][u]);
+        M[2][u] = fma(yl, l23.x, M[2][u]), M[3][u] = fma(yl, l23.y, M[3][u]);
+        M[4][u] = fma(yl, l45.x, M[4][u]), M[5][u] = fma(yl, l45.y, M[5][u]);
+        M[0][u] = fma(yh, h01.x, M[0][u]), M[1][u] = fma(yh, h01.y, M[1][u]);
+        M[2][u] = fma(yh, h23.x, M[2][u]), M[3][u] = fma(yh, h23.y, M[3][u]);
+        M[4][u] = fma(yh, h45.x, M[4][u]), M[5][u] = fma(yh, h45.y, M[5][u]);
+    }
+}
+
 template <int P>
 __device__ __forceinline__ void thermo_finish(const double (&M)[6][P], const double (&Ti)[P], double (&cp)[P], double (&h)[P])
 {
@@ -58,6 +85,7 @@ __device__ __forceinline__ void thermo_finish(const double (&M)[6][P], const dou
     }
 }
 
+template <bool BOTH>
 __global__ void __launch_bounds__(TB, TH_MINB) thermo_kernel(DevTables m, const double *__restrict__ T,
                                                        const double *__restrict__ Y, int64_t n,
                                                        double *__restrict__ cp, double *__restrict__ h)
@@ -85,13 +113,19 @@ __global__ void __launch_bounds__(TB, TH_MINB) thermo_kernel(DevTables m, const 
 #pragma unroll
                 for (int q = 0; q < TH_UNROLL; ++q) {
                     const double y[2] = {y4[q].x, y4[q].y};
-                    thermo_species_step<2>(sm, k + q, y, Tb, M);
+                    if (BOTH)
+                        thermo_species_step_both<2>(sm, k + q, y, Tb, M);
+                    else
+                        thermo_species_step<2>(sm, k + q, y, Tb, M);
                 }
             }
             for (; k < Ns; ++k) {
                 const double2 yy = *reinterpret_cast<const double2 *>(Y + (int64_t)k * n + i);
                 const double y[2] = {yy.x, yy.y};
-                thermo_species_step<2>(sm, k, y, Tb, M);
+                if (BOTH)
+                    thermo_species_step_both<2>(sm, k, y, Tb, M);
+                else
+                    thermo_species_step<2>(sm, k, y, Tb, M);
             }
             double c2[2], h2[2];
             thermo_finish<2>(M, Ti, c2, h2);
@@ -180,7 +214,10 @@ cudaError_t launch_thermo(const DevTables &m, const double *T, const double *Y, 
     const int64_t npair = (n + 1) / 2;
     // TH_MINB blocks of 8 warps per SM; a block walks its share of the point pairs (the table is staged once per block)
     const int64_t blocks = std::min<int64_t>((npair + TB - 1) / TB, 148 * TH_MINB * 4);
-    thermo_kernel<<<(unsigned)blocks, TB, smem, st>>>(m, T, Y, n, cp, h);
+    if (m.thermo_sets == 2)
+        thermo_kernel<true><<<(unsigned)blocks, TB, smem, st>>>(m, T, Y, n, cp, h);
+    else
+        thermo_kernel<false><<<(unsigned)blocks, TB, smem, st>>>(m, T, Y, n, cp, h);
     crf_count_launch();
     return cudaGetLastError();
 }

@@ -258,6 +258,8 @@ PLAN_OVERRIDES = [
     dict(rates_kernel="generic"),                          # one thread per point, libm
     dict(rates_kernel="thread"),                           # one thread per point, product form (default for Ns <= 12)
     dict(transport_kernel="generic"),
+    dict(thermo_sets=1),                                   # crf_thermo: every lane reads the NASA-7 set of its own range
+    dict(thermo_sets=2),                                   # both sets at uniform addresses (the default)
     dict(transport_kernel="small"),
 ]
 
