@@ -76,6 +76,17 @@ def test_argument_errors_need_no_gpu(lib_path):
     t.version = 99
     h = C.c_void_p()
     assert L.crf_mech_create(C.byref(t), C.byref(h)) == -1 and b"version" in L.crf_last_error()
+    # plan options are checked before anything touches a device
+    t = packer.pack(wl.make_mechanism("C1")).as_struct()
+    for field, bad, word in (("transport_TS", 6, b"transport_TS"), ("thermo_sets", 3, b"thermo_sets"), ("reserved", None, b"reserved")):
+        o = binding.PlanOptions()
+        if field == "reserved":
+            o.reserved[0] = 1
+        else:
+            setattr(o, field, bad)
+        assert L.crf_mech_create_ex(C.byref(t), C.byref(o), C.byref(h)) == -1 and word in L.crf_last_error(), field
+    assert L.crf_step_host_static(None, None, None, None, 1, None, None, None, None, None, None, None) == -1
+    assert L.crf_step_host_static_max_points(None) == -1
 
 
 def test_tables_struct_mirrors_header():
