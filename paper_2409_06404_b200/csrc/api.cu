@@ -31,8 +31,23 @@ int fail_cuda(cudaError_t e, const char *where)
 }
 bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
-constexpr int kSlots = 3;          // pipeline depth of crf_step_host
-constexpr int64_t kChunk = 65536;  // points per chunk
+#ifndef CRF_PIPE_SLOTS
+#define CRF_PIPE_SLOTS 3
+#endif
+#ifndef CRF_PIPE_OUT_BYTES
+#define CRF_PIPE_OUT_BYTES (128 << 20)
+#endif
+constexpr int kSlots = CRF_PIPE_SLOTS;  // pipeline depth of crf_step_host
+constexpr int kStoich = 3;              // reactant / product slots of a reaction (crf_tables.reac, prod)
+// points per chunk of crf_step_host: a power of two whose double-precision outputs, 8 (2 Ns + 5) bytes per point, come
+// to about CRF_PIPE_OUT_BYTES per chunk (65536 points at 118 species, 524288 at 21 and fewer): copies long enough to run at the
+// link's rate, enough chunks to overlap the two copy directions and the kernels
+int64_t pipe_chunk_points(int Ns)
+{
+    int64_t c = 16384;
+    while (c < (1 << 19) && 2 * c * 8 * (2 * (int64_t)Ns + 5) <= (int64_t)CRF_PIPE_OUT_BYTES + (CRF_PIPE_OUT_BYTES >> 1)) c *= 2;
+    return c;
+}
 
 }  // namespace
 
@@ -44,8 +59,8 @@ struct crf_mech {
     void *block = nullptr;
     cudaStream_t stream = nullptr;
     // crf_step_host resources (lazy)
-    cudaStream_t pipe_stream[kSlots] = {nullptr, nullptr, nullptr};
-    double *pipe_buf[kSlots] = {nullptr, nullptr, nullptr};
+    cudaStream_t pipe_stream[kSlots] = {};
+    double *pipe_buf[kSlots] = {};
     int64_t pipe_chunk = 0;
 };
 
@@ -110,10 +125,10 @@ int mech_create(const crf_tables *t, const crf_plan_options &opt, crf_mech **out
         thermo_tab[14 * (size_t)k + 12] = Tmid[k];
     }
     std::vector<double> lnA(t->lnA, t->lnA + Nr), beta(t->beta, t->beta + Nr), Ea_R(t->Ea_R, t->Ea_R + Nr), dnu(Nr);
-    std::vector<int16_t> reac(t->reac, t->reac + (size_t)kSlots * Nr), prod(t->prod, t->prod + (size_t)kSlots * Nr);
+    std::vector<int16_t> reac(t->reac, t->reac + (size_t)kStoich * Nr), prod(t->prod, t->prod + (size_t)kStoich * Nr);
     for (int r = 0; r < Nr; ++r) {
         int nf = 0, nb = 0;
-        for (int s = 0; s < kSlots; ++s) {
+        for (int s = 0; s < kStoich; ++s) {
             const int a = reac[(size_t)s * Nr + r], b = prod[(size_t)s * Nr + r];
             if (a >= Ns || b >= Ns || a < -1 || b < -1)
                 return fail(CRF_EINVAL, "crf_mech_create: species index out of range");
@@ -483,7 +498,8 @@ int step_host(const char *name, crf_mech *mech, const double *T, const double *p
         return fail(CRF_EINVAL, std::string(name) + ": the outputs of a call must be given together or all be NULL");
     if (!want_th && !want_ra && !want_tr) return fail(CRF_EINVAL, std::string(name) + ": no output requested");
     const int Ns = mech->dev.Ns;
-    const int64_t chunk = kChunk;
+    // (a call smaller than a chunk sizes the staging buffers for itself; a later, larger call allocates them again)
+    const int64_t chunk = std::min(pipe_chunk_points(Ns), (n + 16383) / 16384 * 16384);
     const size_t rows = 7 + 3 * (size_t)Ns, out_rows = 5 + 2 * (size_t)Ns;
     cudaError_t e;
 #define CRF_TRY(call)                                              \
@@ -515,29 +531,48 @@ int step_host(const char *name, crf_mech *mech, const double *T, const double *p
         CRF_TRY(cudaMemcpyAsync(dp, p + off, w, cudaMemcpyHostToDevice, st))
         CRF_TRY(cudaMemcpy2DAsync(dY, w, Y + off, (size_t)n * sizeof(double), w, Ns, cudaMemcpyHostToDevice, st))
         // one output block of `nrow` rows (leading dimension c on the device, n on the host) back to the host, as doubles or,
-        // rounded once on the device, as floats
+        // rounded once on the device (round32, all blocks before the first copy), as floats
+        auto round32 = [&](double *dev, int nrow) -> cudaError_t {
+            return kF32 ? launch_f64_to_f32(dev, f + (dev - dcp), (int64_t)nrow * c, st) : cudaSuccess;
+        };
         auto back = [&](Out *host, double *dev, int nrow) -> cudaError_t {
             if (!kF32)
                 return cudaMemcpy2DAsync(host + off, (size_t)n * sizeof(Out), dev, w, w, nrow, cudaMemcpyDeviceToHost, st);
             float *fs = f + (dev - dcp);  // (rows are c doubles apart on the device: the float image keeps the same indices)
-            cudaError_t ee = launch_f64_to_f32(dev, fs, (int64_t)nrow * c, st);
-            if (ee != cudaSuccess) return ee;
             return cudaMemcpy2DAsync(host + off, (size_t)n * sizeof(Out), fs, (size_t)c * sizeof(float), (size_t)c * sizeof(float),
                                      nrow, cudaMemcpyDeviceToHost, st);
         };
-        // kernels see a compact chunk: leading dimension c
+        // kernels see a compact chunk: leading dimension c.  All kernels of the chunk first, then all its copies back: a copy
+        // between two kernels would hold the next kernel back (stream order) while the device-to-host engine, which takes
+        // the copies of all slots in issue order, waits for that kernel behind it: the engine idled a third of the time
+        // (C5 end to end 103-111 ms per step; with the copies behind the kernels it streams without gaps)
+        if (want_th) CRF_TRY(launch_thermo(mech->dev, dT, dY, c, dcp, dh, st))
+        if (want_ra) CRF_TRY(launch_rates(mech->dev, dT, dp, dY, c, dom, dq, st))
+        if (want_tr) CRF_TRY(launch_transport(mech->dev, dT, dp, dY, c, dmu, dlam, drD, st))
+        if (kF32) {
+            if (want_th) {
+                CRF_TRY(round32(dcp, 1))
+                CRF_TRY(round32(dh, 1))
+            }
+            if (want_ra) {
+                CRF_TRY(round32(dq, 1))
+                CRF_TRY(round32(dom, Ns))
+            }
+            if (want_tr) {
+                CRF_TRY(round32(dmu, 1))
+                CRF_TRY(round32(dlam, 1))
+                CRF_TRY(round32(drD, Ns))
+            }
+        }
         if (want_th) {
-            CRF_TRY(launch_thermo(mech->dev, dT, dY, c, dcp, dh, st))
             CRF_TRY(back(cp, dcp, 1))
             CRF_TRY(back(h, dh, 1))
         }
         if (want_ra) {
-            CRF_TRY(launch_rates(mech->dev, dT, dp, dY, c, dom, dq, st))
             CRF_TRY(back(qdot, dq, 1))
             CRF_TRY(back(omega, dom, Ns))
         }
         if (want_tr) {
-            CRF_TRY(launch_transport(mech->dev, dT, dp, dY, c, dmu, dlam, drD, st))
             CRF_TRY(back(mu, dmu, 1))
             CRF_TRY(back(lambda, dlam, 1))
             CRF_TRY(back(rhoD, drD, Ns))

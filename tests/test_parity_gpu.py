@@ -186,7 +186,7 @@ def test_step_host_matches_device_calls(binding, oracle_mod):
     """crf_step_host (host buffers, chunked pipeline) gives bit-identical results to the device calls
     on a size that spans several chunks with a ragged last chunk."""
     desc, gm, om = _mech_pair(binding, oracle_mod, "C3")
-    n = 2 * 65536 + 12345
+    n = 2 * 524288 + 12345  # (a chunk of this mechanism is 524288 points)
     st = wl.make_state("C3", n=n)
     gpu = parity.run_gpu(gm, st)
     host = {k: torch.from_numpy(v).pin_memory() for k, v in st.items()}
@@ -202,7 +202,7 @@ def test_step_host_matches_device_calls(binding, oracle_mod):
 def test_step_host_output_groups(binding, oracle_mod):
     """crf_step_host computes and copies only the groups of outputs that are asked for."""
     desc, gm, om = _mech_pair(binding, oracle_mod, "C3")
-    n = 70000  # more than one pipeline chunk
+    n = 600000  # more than one pipeline chunk
     st = wl.make_state("C3", n=n, total=n)
     host = {k: torch.from_numpy(v) for k, v in st.items()}
     full = gm.step_host(host["T"], host["p"], host["Y"])
@@ -219,7 +219,7 @@ def test_step_host_f32_outputs(binding, oracle_mod):
     """crf_step_host_f32: double arithmetic, outputs rounded once to float on the device: every value is the float
     nearest to the double-precision result of crf_step_host (bit for bit), hence within 2^-24 of the oracle."""
     desc, gm, om = _mech_pair(binding, oracle_mod, "C3")
-    n = 66000 + 3
+    n = 540000 + 3  # (two chunks, the second ragged)
     st = wl.make_state("C3", n=n, total=n)
     host = {k: torch.from_numpy(v) for k, v in st.items()}
     full = gm.step_host(host["T"], host["p"], host["Y"])
