@@ -31,21 +31,16 @@ int fail_cuda(cudaError_t e, const char *where)
 }
 bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
-#ifndef CRF_PIPE_SLOTS
-#define CRF_PIPE_SLOTS 3
-#endif
-#ifndef CRF_PIPE_OUT_BYTES
-#define CRF_PIPE_OUT_BYTES (128 << 20)
-#endif
-constexpr int kSlots = CRF_PIPE_SLOTS;  // pipeline depth of crf_step_host
+constexpr int kSlots = 3;                       // pipeline depth of crf_step_host (four measured: no difference)
+constexpr int64_t kPipeOutBytes = 128 << 20;    // output bytes of a chunk to aim for (64 MB, 256 MB measured: no difference)
 constexpr int kStoich = 3;              // reactant / product slots of a reaction (crf_tables.reac, prod)
 // points per chunk of crf_step_host: a power of two whose double-precision outputs, 8 (2 Ns + 5) bytes per point, come
-// to about CRF_PIPE_OUT_BYTES per chunk (65536 points at 118 species, 524288 at 21 and fewer): copies long enough to run at the
+// to about kPipeOutBytes per chunk (65536 points at 118 species, 524288 at 21 and fewer): copies long enough to run at the
 // link's rate, enough chunks to overlap the two copy directions and the kernels
 int64_t pipe_chunk_points(int Ns)
 {
     int64_t c = 16384;
-    while (c < (1 << 19) && 2 * c * 8 * (2 * (int64_t)Ns + 5) <= (int64_t)CRF_PIPE_OUT_BYTES + (CRF_PIPE_OUT_BYTES >> 1)) c *= 2;
+    while (c < (1 << 19) && 2 * c * 8 * (2 * (int64_t)Ns + 5) <= kPipeOutBytes + (kPipeOutBytes >> 1)) c *= 2;
     return c;
 }
 
