@@ -274,6 +274,12 @@ def other_path(args, mech, dev, out, n, name, world, rank, local, barrier, flush
         alg_bytes = 8 * 2 * (Ns + 2) + 8 * 2 * (Ns + 1)
         sep_name, sep_note = "separate_calls", "3 axpy + 2 crf_production_rates + 2 quotient kernels (torch elementwise)"
 
+        def with_base():  # the base values in hand (what an integrator has): only the perturbed state is evaluated
+            mech.production_rates_jv_base(dev["T"], dev["p"], dev["Y"], v["T"], v["p"], v["Y"], sigma,
+                                          out["omega"], out["qdot"], out=(Jo, Jq))
+        extra = ("with_base", with_base, "crf_production_rates_jv_base: omega(y), qdot(y) given, one state evaluated",
+                 w_ra["F"], 8 * 2 * (Ns + 2) + 8 * 2 * (Ns + 1))
+
     K = max(args.steps, 1)
 
     def timed(fn):
@@ -300,6 +306,11 @@ def other_path(args, mech, dev, out, n, name, world, rank, local, barrier, flush
     launches = (binding.launch_count() - launches0) * K // (K + max(args.warmup, 3))
     clock_info = clocks.stop() if clocks else None
     sep_ms, sep_med, sep_best = timed(separate)
+    extra_out = None
+    if args.path == "jv":
+        x_ms, x_med, x_best = timed(extra[1])
+        extra_out = {"ms_per_step": x_ms, "ms_median": x_med, "ms_best": x_best, "what": extra[2],
+                     "frac_of_fp64_roofline": extra[3] * n / (rooflines.FP64_PEAK_TFLOPS * 1e12) / (x_ms * 1e-3)}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -322,6 +333,8 @@ def other_path(args, mech, dev, out, n, name, world, rank, local, barrier, flush
             "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": None,
             sep_name: {"ms_per_step": sep_ms, "ms_median": sep_med, "ms_best": sep_best, "what": sep_note,
                        "fused_over_separate": ms / sep_ms}}
+    if extra_out:
+        line[extra[0]] = extra_out
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

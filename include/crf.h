@@ -177,6 +177,18 @@ int crf_production_rates_jv(const crf_mech *mech, const double *T, const double 
                             const double *dp, const double *dY, double sigma, int64_t n, double *omega, double *qdot,
                             double *Jomega, double *Jqdot);
 
+/* The same difference quotient when omega(y) and qdot(y) are known already, which is how an integrator calls it: CVODE's
+ * matrix-free Newton-Krylov iteration forms J v = (f(y + sigma v) - f(y)) / sigma with f(y) in hand, and
+ * the Jacobian-vector products are most of the right-hand-side evaluations of a step.  omega[Ns*n] and
+ * qdot[n] are INPUTS here (the values crf_production_rates returned for (T, p, Y)); only the perturbed state is
+ * evaluated, at the cost of one crf_production_rates call:
+ *   Jomega = (omega(y') - omega) (1/sigma),   Jqdot = (qdot(y') - qdot) (1/sigma),   y' as in crf_production_rates_jv
+ * (bit for bit what crf_production_rates_jv returns for the same base values).  dp may be NULL.  CRF_EUNSUPPORTED for a
+ * mechanism that runs a fall-back kernel. */
+int crf_production_rates_jv_base(const crf_mech *mech, const double *T, const double *p, const double *Y, const double *dT,
+                                 const double *dp, const double *dY, double sigma, int64_t n, const double *omega,
+                                 const double *qdot, double *Jomega, double *Jqdot);
+
 /* The element-local spectral-element diffusion operator on what crf_rhs_pointwise emits: "diffusion"
  * is the most expensive kernel of the paper's right-hand side.  The fields live on nel hexahedral
  * elements of polynomial order 7: n = 512 nel points, node (i, j, k) of element e at

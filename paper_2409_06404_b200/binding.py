@@ -20,6 +20,7 @@ _lib = None
 EXPORTS = ("crf_mech_create", "crf_mech_destroy", "crf_mech_set_stream", "crf_mech_num_species",
            "crf_mech_num_reactions", "crf_thermo", "crf_thermo_species", "crf_production_rates",
            "crf_mix_transport", "crf_rhs_pointwise", "crf_production_rates_pair", "crf_production_rates_jv",
+           "crf_production_rates_jv_base",
            "crf_sem_diffusion", "crf_step_host", "crf_step_host_f32", "crf_step_host_static",
            "crf_step_host_static_max_points", "crf_last_error")
 EXPORTS_DIAG = ("crf_mech_create_ex", "crf_mech_plan_info", "crf_fp64_probe", "crf_launch_count",
@@ -75,6 +76,7 @@ def lib() -> C.CDLL:
         L.crf_rhs_pointwise.argtypes = [vp, dp, dp, dp, i64] + [dp] * 10
         L.crf_production_rates_pair.argtypes = [vp] + [dp] * 6 + [i64] + [dp] * 4
         L.crf_production_rates_jv.argtypes = [vp] + [dp] * 6 + [C.c_double, i64] + [dp] * 4
+        L.crf_production_rates_jv_base.argtypes = [vp] + [dp] * 6 + [C.c_double, i64] + [dp] * 4
         L.crf_sem_diffusion.argtypes = [vp] + [dp] * 6 + [i64, dp, dp]
         L.crf_step_host.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
         L.crf_step_host_f32.argtypes = [vp, dp, dp, dp, i64] + [dp] * 7
@@ -237,6 +239,18 @@ class Mechanism:
             self._h, _dev(T, (n,)), _dev(p, (n,)), _dev(Y, (self.Ns, n)), _dev(dT, (n,)), _dev(dp),
             _dev(dY, (self.Ns, n)), float(sigma), n, _dev(out[0]), _dev(out[1]), _dev(out[2], (self.Ns, n)),
             _dev(out[3], (n,))))
+        return out
+
+    def production_rates_jv_base(self, T, p, Y, dT, dp, dY, sigma, omega, qdot, out=None):
+        """``crf_production_rates_jv_base``: (Jomega, Jqdot) against the given base values omega(y), qdot(y) (inputs)."""
+        n = T.numel()
+        if out is None:
+            out = (torch.empty_like(Y), torch.empty_like(T))
+        self._sync_stream()
+        _check(lib().crf_production_rates_jv_base(
+            self._h, _dev(T, (n,)), _dev(p, (n,)), _dev(Y, (self.Ns, n)), _dev(dT, (n,)), _dev(dp),
+            _dev(dY, (self.Ns, n)), float(sigma), n, _dev(omega, (self.Ns, n)), _dev(qdot, (n,)),
+            _dev(out[0], (self.Ns, n)), _dev(out[1], (n,))))
         return out
 
     def sem_diffusion(self, h3, T, Wbar, Y, lam, rhoD, dY=None, dT=None):

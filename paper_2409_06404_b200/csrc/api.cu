@@ -424,6 +424,33 @@ int crf_production_rates_jv(const crf_mech *mech, const double *T, const double 
     return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_production_rates_jv");
 }
 
+int crf_production_rates_jv_base(const crf_mech *mech, const double *T, const double *p, const double *Y, const double *dT,
+                                 const double *dp, const double *dY, double sigma, int64_t n, const double *omega,
+                                 const double *qdot, double *Jomega, double *Jqdot)
+{
+    CRF_CHECK_COMMON("crf_production_rates_jv_base")
+    if (!T || !p || !Y || !dT || !dY || !omega || !qdot || !Jomega || !Jqdot)
+        return fail(CRF_EINVAL, "crf_production_rates_jv_base: null pointer");
+    if (!(sigma != 0.0) || !std::isfinite(sigma))
+        return fail(CRF_EINVAL, "crf_production_rates_jv_base: sigma must be finite and non-zero");
+    for (const void *q : {(const void *)T, (const void *)p, (const void *)Y, (const void *)dT, (const void *)dp,
+                          (const void *)dY, (const void *)omega, (const void *)qdot, (const void *)Jomega, (const void *)Jqdot})
+        if (misaligned(q)) return fail(CRF_EINVAL, "crf_production_rates_jv_base: pointers must be 16-byte aligned");
+    // (the kernels read the base values through the output slots of RatesIO and do not write them in this mode)
+    RatesIO io = rates_io(T, p, Y, const_cast<double *>(omega), const_cast<double *>(qdot));
+    io.T2 = dT, io.Y2 = dY, io.omega2 = Jomega, io.qdot2 = Jqdot, io.sigma = sigma, io.inv_sigma = 1.0 / sigma, io.mode = 4;
+    io.p2 = dp ? dp : p, io.sigma_p = dp ? sigma : 0.0;
+    cudaError_t e;
+    if (rates_thread_tm_serves(mech->dev, io))
+        e = launch_rates_thread_io(mech->dev, io, n, mech->stream);
+    else if (mech->dev.rg.W > 0)
+        e = launch_rates_group(mech->dev, io, n, mech->stream);
+    else
+        return fail(CRF_EUNSUPPORTED, "crf_production_rates_jv_base: this mechanism runs a fall-back kernel (use "
+                                      "crf_production_rates on a perturbed copy)");
+    return e == cudaSuccess ? CRF_OK : fail_cuda(e, "crf_production_rates_jv_base");
+}
+
 int crf_rhs_pointwise(const crf_mech *mech, const double *T, const double *p, const double *Y, int64_t n, double *omega,
                       double *qdot, double *cp, double *h, double *cpk, double *rho, double *Wbar, double *mu,
                       double *lambda, double *rhoD)

@@ -71,7 +71,8 @@ using crf::load_row;
 using crf::store_row;
 
 // input row of the lane: MODE 0 the PPL adjacent points of `a`; MODE 1 (a[i], b[i]); MODE 2 (a[i], a[i] + sigma b[i]),
-// one rounding per operation so that the perturbed state is the one a host forms
+// one rounding per operation so that the perturbed state is the one a host forms; MODE 4: the PPL adjacent points of
+// a + sigma b (the perturbed state only: the base values of the quotient are given)
 template <int PPL, int MODE>
 __device__ __forceinline__ void in_row(const RatesIO &io, const double *__restrict__ a, const double *__restrict__ b,
                                        double sigma, int64_t i0, int64_t n, bool vec, double (&v)[PPL])
@@ -80,18 +81,35 @@ __device__ __forceinline__ void in_row(const RatesIO &io, const double *__restri
         load_row<PPL>(a, i0, n, vec, v);
         return;
     }
+    if (MODE == 4) {
+        double vb[PPL];
+        load_row<PPL>(a, i0, n, vec, v);
+        load_row<PPL>(b, i0, n, vec, vb);
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) v[u] = __dadd_rn(v[u], __dmul_rn(sigma, vb[u]));
+        return;
+    }
     const int64_t i = min(i0, n - 1);
     const double va = a[i], vb = b[i];
     v[0] = va;
     v[PPL - 1] = MODE == 1 ? vb : __dadd_rn(va, __dmul_rn(sigma, vb));
 }
-// output rows: MODE 0 -> a; MODE 1: v[0] -> a, v[1] -> b; MODE 2: v[0] -> a (if given), (v[1] - v[0]) (1/sigma) -> b
+// output rows: MODE 0 -> a; MODE 1: v[0] -> a, v[1] -> b; MODE 2: v[0] -> a (if given), (v[1] - v[0]) (1/sigma) -> b;
+// MODE 4: (v - a) (1/sigma) -> b, a holding the base values (read only)
 template <int PPL, int MODE>
 __device__ __forceinline__ void out_rows(const RatesIO &io, double *__restrict__ a, double *__restrict__ b, int64_t off,
                                          int64_t i0, int64_t n, bool vec, const double (&v)[PPL])
 {
     if (MODE == 0) {
         store_row<PPL>(a + off, i0, n, vec, v);
+        return;
+    }
+    if (MODE == 4) {
+        double base[PPL], o[PPL];
+        load_row<PPL>(a + off, i0, n, vec, base);
+#pragma unroll
+        for (int u = 0; u < PPL; ++u) o[u] = __dmul_rn(__dsub_rn(v[u], base[u]), io.inv_sigma);
+        store_row<PPL>(b + off, i0, n, vec, o);
         return;
     }
     if (i0 >= n) return;
@@ -357,7 +375,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     // states of ONE grid point, so tables, records and lists are read once for both evaluations
     constexpr int mode = MODE == 3 ? 0 : MODE;
     constexpr bool EXT = MODE == 3;
-    const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * (mode == 0 ? PPL : 1);
+    const int64_t i0 = ((int64_t)blockIdx.x * 32 + lane) * (mode == 0 || mode == 4 ? PPL : 1);
     const bool vec = (n & 1) == 0;
     Ctx<PPL> c;
     double pi[PPL];
@@ -596,14 +614,15 @@ cudaError_t launch_k(const DevTables &m, const RatesIO &io, int64_t n, cudaStrea
     const bool emit = io.cp || io.h || io.cpk || io.rho || io.Wbar;
     void (*kernel)(DevTables, RatesIO, int64_t) = rates_group_kernel<W, PPL, MAXOWN, TM, 0>;
     if (io.mode == 0 && emit) kernel = rates_group_kernel<W, PPL, MAXOWN, TM, 3>;
-    if (io.mode != 0) {
+    if (io.mode == 4) kernel = rates_group_kernel<W, PPL, MAXOWN, TM, 4>;
+    if (io.mode == 1 || io.mode == 2) {
         if (PPL != 2) return cudaErrorInvalidValue;
         // (instantiated for two points per lane only)
         kernel = io.mode == 1 ? rates_group_kernel<W, 2, MAXOWN, TM, 1> : rates_group_kernel<W, 2, MAXOWN, TM, 2>;
     }
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const int64_t per_block = io.mode == 0 ? 32 * PPL : 32;
+    const int64_t per_block = io.mode == 0 || io.mode == 4 ? 32 * PPL : 32;
     kernel<<<(unsigned)((n + per_block - 1) / per_block), 32 * W, smem, st>>>(m, io, n);
     crf_count_launch();
     return cudaGetLastError();
@@ -635,7 +654,7 @@ size_t rates_group_dynamic_smem(const DevTables &m)
 // io.mode 1 and 2 need a plan with two points per lane (the two states of a grid point share a lane)
 cudaError_t launch_rates_group(const DevTables &m, const RatesIO &io, int64_t n, cudaStream_t st)
 {
-    if (io.mode != 0 && m.rg.PPL != 2) return cudaErrorInvalidValue;
+    if ((io.mode == 1 || io.mode == 2) && m.rg.PPL != 2) return cudaErrorInvalidValue;
     switch (m.rg.W * 10 + m.rg.PPL) {
     case 41: return launch_wp<4, 1>(m, io, n, st);
     case 42: return launch_wp<4, 2>(m, io, n, st);

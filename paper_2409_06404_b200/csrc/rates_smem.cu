@@ -374,6 +374,7 @@ __global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, Rate
         const unsigned tom = tmq + 4u * (Ns + 1);  // omega of this state (the columns are reused by the second state)
         // the state: mode 1 = the second set of arrays, mode 2 = perturbed in place (multiply, then add: one rounding each)
         auto in = [&](const double *a, const double *b, double sg, int64_t idx) {
+            if (MODE == 4) return __dadd_rn(a[idx], __dmul_rn(sg, b[idx]));  // (the perturbed state only: the base is given)
             if (st == 0 || MODE == 0 || MODE == 3) return a[idx];
             return MODE == 1 ? b[idx] : __dadd_rn(a[idx], __dmul_rn(sg, b[idx]));
         };
@@ -465,7 +466,9 @@ __global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, Rate
                 // (mode 2: omega of the base state waits in global memory, in `omega` if the caller wants it, else in the
                 // quotient's own row, and is read back by the same thread when the second state is done)
                 double *base = MODE == 2 && !io.omega ? io.omega2 : io.omega;
-                if (st == 0)
+                if (MODE == 4)
+                    io.omega2[o] = __dmul_rn(__dsub_rn(w, io.omega[o]), io.inv_sigma);
+                else if (st == 0)
                     base[o] = w;
                 else if (MODE == 1)
                     io.omega2[o] = w;
@@ -487,7 +490,9 @@ __global__ void __launch_bounds__(RT_B) rates_thread_tm_kernel(DevTables m, Rate
         if (i < n) {
             const double q = qd * (CRF_R_GAS * Tu);
             double *base = MODE == 2 && !io.qdot ? io.qdot2 : io.qdot;
-            if (st == 0) {
+            if (MODE == 4) {
+                io.qdot2[i] = __dmul_rn(__dsub_rn(q, io.qdot[i]), io.inv_sigma);
+            } else if (st == 0) {
                 base[i] = q;
                 if (MODE == 3 && io.cp) io.cp[i] = cpm * CRF_R_GAS;
                 if (MODE == 3 && io.h) io.h[i] = hm * (CRF_R_GAS * Tu);
@@ -516,6 +521,7 @@ cudaError_t launch_thread_tm(const DevTables &m, const RatesIO &io, int64_t n, c
     if (io.mode == 0 && emit) kernel = rates_thread_tm_kernel<3>;
     if (io.mode == 1) kernel = rates_thread_tm_kernel<1>;
     if (io.mode == 2) kernel = rates_thread_tm_kernel<2>;
+    if (io.mode == 4) kernel = rates_thread_tm_kernel<4>;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kernel<<<(unsigned)((n + RT_B - 1) / RT_B), RT_B, smem, st>>>(m, io, n, cols);

@@ -158,6 +158,46 @@ def test_jv_difference_quotient(binding, oracle_mod, name, sigma):
     assert np.max(np.abs(Jo3.cpu().numpy() - ref3["Jomega"]) / (parity.RATE_TOL * ref3["S_Jomega"] + 1e-30 / abs(sigma))) <= 1.0
 
 
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+def test_jv_against_a_given_base(binding, oracle_mod, name):
+    """crf_production_rates_jv_base: omega(y), qdot(y) are inputs (what an integrator has in hand), only
+    the perturbed state is evaluated: bit for bit the quotient of crf_production_rates_jv for the same base values, within
+    tolerance of the oracle's quotient, also under a plan with one point per lane (which the two-state call declines)."""
+    desc = wl.make_mechanism(name)
+    gm, om = binding.Mechanism(desc), oracle_mod.Oracle(desc)
+    n = SMALL_N[name] + 1  # odd: the ragged tail of the two-points-per-lane rows
+    st = wl.make_state(name, n=n, total=n)
+    rng = np.random.default_rng(43)
+    v = dict(dT=st["T"] * rng.uniform(-1, 1, n), dp=st["p"] * rng.uniform(-1, 1, n),
+             dY=st["Y"] * rng.uniform(-1, 1, st["Y"].shape))
+    d, dv = parity.to_dev(st), parity.to_dev(v)
+    sigma = 1e-6
+    om_b, qd_b, Jo, Jq = gm.production_rates_jv(d["T"], d["p"], d["Y"], dv["dT"], dv["dp"], dv["dY"], sigma)
+    om_s, qd_s = gm.production_rates(d["T"], d["p"], d["Y"])
+    assert torch.equal(om_s, om_b) and torch.equal(qd_s, qd_b)
+    keep = (om_s.clone(), qd_s.clone())
+    Jo4, Jq4 = gm.production_rates_jv_base(d["T"], d["p"], d["Y"], dv["dT"], dv["dp"], dv["dY"], sigma, om_s, qd_s)
+    assert torch.equal(Jo4, Jo) and torch.equal(Jq4, Jq)
+    assert torch.equal(om_s, keep[0]) and torch.equal(qd_s, keep[1])  # the base values are inputs: untouched
+    ref = om.production_rates_jv(st["T"], st["p"], st["Y"], v["dT"], v["dp"], v["dY"], sigma)
+    for got, key, sk in ((Jo4, "Jomega", "S_Jomega"), (Jq4, "Jqdot", "S_Jqdot")):
+        assert np.max(np.abs(got.cpu().numpy() - ref[key]) / (parity.RATE_TOL * ref[sk] + 1e-30 / abs(sigma))) <= 1.0, (name, key)
+    # no pressure perturbation
+    Jo5, _ = gm.production_rates_jv_base(d["T"], d["p"], d["Y"], dv["dT"], None, dv["dY"], sigma, om_s, qd_s)
+    ref5 = om.production_rates_jv(st["T"], st["p"], st["Y"], v["dT"], np.zeros(n), v["dY"], sigma)
+    assert np.max(np.abs(Jo5.cpu().numpy() - ref5["Jomega"]) / (parity.RATE_TOL * ref5["S_Jomega"] + 1e-30 / abs(sigma))) <= 1.0
+    # one point per lane in the warp-group kernel
+    g1 = binding.Mechanism(desc, options=dict(rates_kernel="group", rates_PPL=1))
+    b1 = g1.production_rates(d["T"], d["p"], d["Y"])
+    Jo6, Jq6 = g1.production_rates_jv_base(d["T"], d["p"], d["Y"], dv["dT"], dv["dp"], dv["dY"], sigma, *b1)
+    for got, key, sk in ((Jo6, "Jomega", "S_Jomega"), (Jq6, "Jqdot", "S_Jqdot")):
+        assert np.max(np.abs(got.cpu().numpy() - ref[key]) / (parity.RATE_TOL * ref[sk] + 1e-30 / abs(sigma))) <= 1.0, (name, key, "PPL=1")
+    # a fall-back kernel declines
+    g2 = binding.Mechanism(desc, options=dict(rates_kernel="staged"))
+    with pytest.raises(binding.CrfError, match="fall-back"):
+        g2.production_rates_jv_base(d["T"], d["p"], d["Y"], dv["dT"], dv["dp"], dv["dY"], sigma, *b1)
+
+
 def test_new_calls_reject_bad_arguments(binding):
     desc = wl.make_mechanism("C1")
     gm = binding.Mechanism(desc)
