@@ -529,6 +529,23 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
     double qd[PPL], cpm[PPL], hm[PPL];
 #pragma unroll
     for (int u = 0; u < PPL; ++u) qd[u] = cpm[u] = hm[u] = 0.0;
+    if (mode == 4) {  // the quotient against given base values: their rows are read in one batch, then om -> (om - base) / sigma
+        double base[MAXOWN][PPL];
+#pragma unroll
+        for (int s = 0; s < MAXOWN; ++s) {
+            const int k = __ldg(rg.own + warp * MAXOWN + s);
+            load_row<PPL>(io.omega + (int64_t)max(k, 0) * n, i0, n, vec, base[s]);
+        }
+#pragma unroll
+        for (int s = 0; s < MAXOWN; ++s)
+#pragma unroll
+            for (int u = 0; u < PPL; ++u) base[s][u] = __dmul_rn(__dsub_rn(om[s][u], base[s][u]), io.inv_sigma);
+#pragma unroll
+        for (int s = 0; s < MAXOWN; ++s) {
+            const int k = __ldg(rg.own + warp * MAXOWN + s);
+            if (k >= 0) store_row<PPL>(io.omega2 + (int64_t)k * n, i0, n, vec, base[s]);
+        }
+    }
 #pragma unroll
     for (int s = 0; s < MAXOWN; ++s) {
         const int k = __ldg(rg.own + warp * MAXOWN + s);
@@ -541,7 +558,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
                 hk[u] = nasa_eval<false>(h, c.T[u], c.rT[u], 0.0, Tmid);
                 qd[u] = fma(-hk[u], om[s][u], qd[u]);
             }
-            out_rows<PPL, mode>(io, io.omega, io.omega2, (int64_t)k * n, i0, n, vec, om[s]);
+            if (mode != 4) out_rows<PPL, mode>(io, io.omega, io.omega2, (int64_t)k * n, i0, n, vec, om[s]);
             if (emit) {
                 // crf_rhs_pointwise: c_pk/R from the h/(RT) set (a_i = (i + 1) c_i), mixture c_p and h; the Y row is
                 // read again (it was consumed by the species this warp handled in the prologue, not the ones it owns)
