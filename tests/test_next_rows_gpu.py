@@ -249,7 +249,10 @@ def test_next_rows_at_full_size_sampled(binding, oracle_mod, name):
     assert np.max(np.abs(take(Jo) - ref["Jomega"]) / (parity.RATE_TOL * ref["S_Jomega"] + 1e-30 / sigma)) <= 1.0
     assert np.max(np.abs(take(Jq) - ref["Jqdot"]) / (parity.RATE_TOL * ref["S_Jqdot"] + 1e-30 / sigma)) <= 1.0
     assert bool(torch.isfinite(Jo).all())
-    del Jo, v
+    # crf_production_rates_jv_base on the whole field: the same quotient, bit for bit, from the base values of the plain call
+    Jo2, Jq2 = gm.production_rates_jv_base(d["T"], d["p"], d["Y"], v["T"], v["p"], v["Y"], sigma, rhs["omega"], rhs["qdot"])
+    assert torch.equal(Jo2, Jo) and torch.equal(Jq2, Jq)
+    del Jo, Jo2, v
 
     # crf_sem_diffusion on every element, sampled elements against the oracle (the operator is element-local)
     nel = n // 512
